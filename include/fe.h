@@ -1,0 +1,127 @@
+/* fe.h -- C ABI of libfe_b200: the TDGL hot path of arxiv/paper_2605_28800 (PETASPIN_microelectrics)
+ * on one B200 (sm_100a).
+ *
+ * What the library computes (citations: PAPER.md = /root/reference/PAPER.md line, equation):
+ *   dP_i/dt = L * active * ( E_Land + E_Grad + E_Elec + E_Ext )_i          PAPER.md:33-35 (Eq. 1)
+ *   E_Land  = -d f_Land / dP, f_Land = Eq. 3 (+ four 8th-order slots)      PAPER.md:41-47 (Eq. 3)
+ *   E_Grad  = -(1/V) dF_Grad,h/dP, F_Grad = Eq. 4 on the cell grid         PAPER.md:53-60 (Eq. 4)
+ *   E_Elec  = -(1/(eps0 epsB)) sum_r' K(r-r') P(r')  (cell-averaged dipolar tensor, P = 0 outside,
+ *             evaluated as a zero-padded FFT convolution)                  PAPER.md:66-76 (Eq. 5-6), 115
+ *   E_Ext   = uniform applied field per simulation                         PAPER.md:78-81 (Eq. 7)
+ * over a batch of independent simulations that share geometry             PAPER.md:117.
+ * DESIGN.md lists every reading taken where the paper is silent (stencil, periodic axes, tensor).
+ *
+ * Conventions
+ *   Memory.   Every pointer named dev_* / P / dPdt / the workspace is DEVICE memory owned by the caller
+ *             (e.g. a torch tensor); every other pointer is HOST memory.  The library allocates only
+ *             a few kB of device memory for coefficient and index tables (freed by fe_destroy_grid).
+ *   Layout.   State arrays are [batch][3][nz][ny][nx], x fastest, contiguous, 16-byte aligned, of the
+ *             grid's dtype (double for FE_F64, float for FE_F32).  Material map: uint8 [nz][ny][nx].
+ *   Streams.  `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  fe_rhs and
+ *             fe_step enqueue work and return; fe_precompute_tensor, fe_energy and fe_get_tensor
+ *             synchronise the stream before returning.
+ *   Errors.   Every call returns fe_status; nothing throws or aborts.  fe_last_error() returns the
+ *             text of the last failure on the calling thread.
+ *   Units.    The library is unit-agnostic; it evaluates the formulas above with the numbers given.
+ */
+#ifndef FE_B200_H
+#define FE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fe_grid fe_grid;   /* opaque; created by fe_create_grid, freed by fe_destroy_grid */
+
+typedef enum {
+    FE_OK = 0,
+    FE_EINVAL = 1,      /* bad argument (sizes not a power of two in 4..1024, batch < 1, dx <= 0, ...) */
+    FE_ENOMEM = 2,      /* workspace too small / allocation of the small tables failed               */
+    FE_ECUDA = 3,       /* a CUDA call failed; text in fe_last_error()                              */
+    FE_ESTATE = 4,      /* call order: no workspace bound, tensor not precomputed, material unset    */
+    FE_ENONFINITE = 5   /* fe_energy found NaN/Inf                                                  */
+} fe_status;
+
+enum { FE_F64 = 0, FE_F32 = 1 };
+enum { FE_TERM_LANDAU = 1, FE_TERM_GRADIENT = 2, FE_TERM_ELEC = 4, FE_TERM_EXT = 8, FE_TERM_ALL = 15 };
+enum { FE_EULER = 0, FE_HEUN = 1, FE_RK4 = 2 };   /* PAPER.md:117-119; RK4 = BASELINE.json config 2 */
+
+/* Geometry of the batch (PAPER.md:113 uniform cells; PAPER.md:117 batch). */
+typedef struct {
+    int32_t nx, ny, nz;        /* cells per axis; each a power of two in [4, 1024]                  */
+    double  dx, dy, dz;        /* cell size > 0                                                     */
+    int32_t periodic[3];       /* per axis: 0 = open (vacuum outside, FFT zero-padded to 2n), 1 = periodic */
+    int32_t pbc_images[3];     /* R >= 0 image cells summed on each side of a periodic axis         */
+    int32_t batch;             /* B >= 1 independent simulations                                    */
+    int32_t dtype;             /* FE_F64 or FE_F32: type of every state array and of the arithmetic */
+    int32_t n_materials;       /* M in 1..255: rows of the per-member coefficient table             */
+    int32_t zero_mode;         /* != 0: with exactly two periodic axes, fix each plane sum of the
+                                  kernel to the infinite-film value (reading A4)          */
+} fe_grid_desc;
+
+/* Landau coefficients of one material (Eq. 3, Table 1). a1 per axis. */
+typedef struct {
+    double  a1[3];
+    double  a11, a12, a111, a112, a123;
+    double  a1111, a1112, a1122, a1123;   /* 8th-order cubic-symmetry slots; 0 for the paper's tables */
+    int32_t active;                       /* 0 = vacuum cell: P stays 0, no gradient bonds to it     */
+} fe_landau;
+
+/* Per-simulation scalars: Eq. 4 coefficients, eps0*epsB of Eq. 6, kinetic coefficient L of Eq. 1. */
+typedef struct { double G11, G12, G44, G44p; double eps0, epsB, L; } fe_global;
+
+/* Create / destroy.  *out is set only on FE_OK. */
+fe_status fe_create_grid(const fe_grid_desc* desc, fe_grid** out);
+fe_status fe_destroy_grid(fe_grid* g);
+
+/* Device scratch the caller must provide (spectra, tensor spectrum, stage buffers). */
+size_t    fe_workspace_bytes(const fe_grid* g);
+/* dev must be 256-byte aligned device memory of at least fe_workspace_bytes(g); borrowed until
+ * fe_destroy_grid or the next fe_bind_workspace (which invalidates a precomputed tensor). */
+fe_status fe_bind_workspace(fe_grid* g, void* dev, size_t bytes);
+
+/* Coefficients.  member = -1 sets every batch member.  May be called between steps at any time
+ * (no tensor recompute needed); takes effect at the next fe_rhs/fe_step/fe_energy call. */
+fe_status fe_set_material(fe_grid* g, int32_t member, int32_t material_id, const fe_landau* m);
+fe_status fe_set_global(fe_grid* g, int32_t member, const fe_global* gl);
+fe_status fe_set_external_field(fe_grid* g, int32_t member, const double E[3]);
+/* dev_map: uint8 [nz][ny][nx] material id per cell, shared by the batch; NULL = all cells material 0.
+ * Borrowed (not copied). */
+fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map);
+
+/* a0: cell-averaged dipolar tensor K_ij(d) on the padded box and its real spectrum (once per
+ * geometry).  PAPER.md:76,115; readings A3, A4. */
+fe_status fe_precompute_tensor(fe_grid* g, void* cuda_stream);
+
+/* a1-a4: dPdt = RHS(P) for the terms in the bitmask.  P and dPdt must not alias. */
+fe_status fe_rhs(fe_grid* g, const void* P, void* dPdt, uint32_t terms, void* cuda_stream);
+
+/* a5: nsteps explicit steps of size dt, in place on P.  Coefficients and E_Ext are constant during
+ * the call. */
+fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int32_t integrator,
+                  uint32_t terms, void* cuda_stream);
+
+/* a6: host_out[b][8] = { F_Land, F_Grad, F_Elec, F_Ext, F_tot, <Px>, <Py>, <Pz> } for the terms in
+ * the bitmask (Eq. 2, 5, 7); energies are densities times cell volume summed over cells, means are
+ * over active cells.  Returns FE_ENONFINITE if any value is NaN/Inf (host_out is still written). */
+fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double* host_out, void* cuda_stream);
+
+/* Test hooks. */
+/* host_out: [6][mz][my][mx] doubles (xx yy zz xy xz yz), the real-space kernel on the circular padded
+ * box (m = 2n open, n periodic; entry at index (d mod m) holds K(d)). */
+fe_status fe_get_tensor(fe_grid* g, double* host_out, void* cuda_stream);
+/* padded box size per axis (mx, my, mz) */
+fe_status fe_padded_dims(const fe_grid* g, int32_t out[3]);
+/* number of kernel launches issued by this grid since creation (bench.py's gpu_launches claim) */
+uint64_t  fe_launch_count(const fe_grid* g);
+
+const char* fe_last_error(void);
+const char* fe_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FE_B200_H */

@@ -1,0 +1,586 @@
+// fe_api.cu -- the C ABI of libfe_b200 (include/fe.h): argument checking, workspace layout, the
+// sequence of kernel launches of one RHS evaluation and the explicit
+// integrators (a5).  All arithmetic of the method is in the kernels.
+#include "../../include/fe.h"
+#include "fe_internal.h"
+
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+#include <new>
+#include <vector>
+
+using namespace fe;
+
+static thread_local char g_err[512] = "";
+
+static fe_status fail(fe_status s, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return s;
+}
+
+#define FE_CUDA(call)                                                                          \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) return fail(FE_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+struct fe_grid {
+    fe_grid_desc desc;
+    Geometry geo;
+    bool f32;
+    size_t rsz, csz;                 // bytes of a real / complex element of the state dtype
+    int64_t N;
+    // host mirrors of the coefficient tables
+    std::vector<DevLandau> h_mats;   // [B][nmat]
+    std::vector<uint8_t> mat_set;
+    std::vector<DevMember> h_members;
+    std::vector<fe_global> h_globals;
+    std::vector<uint8_t> glob_set;
+    bool dirty;
+    int mixed;
+    // small device tables owned by the library
+    unsigned char* d_small;
+    DevLandau* d_mats;
+    DevMember* d_members;
+    double* d_eout;
+    FftCtx ctx;                      // state dtype
+    FftCtx ctx64;                    // fp64 (tensor precompute)
+    const uint8_t* map;
+    // workspace (borrowed)
+    unsigned char* ws;
+    size_t ws_bytes;
+    size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_part, o_box, o_Sbox, total_bytes;
+    int nblk;
+    bool tensor_ready;
+    uint64_t launches;
+};
+
+static AxisPlan make_plan(int M)
+{
+    AxisPlan p;
+    memset(&p, 0, sizeof(p));
+    p.M = M;
+    int L = 0;
+    while ((1 << L) < M) ++L;
+    p.logM = L;
+    int n8 = L / 3, rem = L % 3, k = 0;
+    if (rem == 1 && n8 >= 1) {
+        for (int i = 0; i < n8 - 1; ++i) p.radix[k++] = 8;
+        p.radix[k++] = 4;
+        p.radix[k++] = 4;
+    } else {
+        for (int i = 0; i < n8; ++i) p.radix[k++] = 8;
+        if (rem == 2) p.radix[k++] = 4;
+        if (rem == 1) p.radix[k++] = 2;
+    }
+    p.nst = k;
+    return p;
+}
+
+// position p after the forward (DIF) stages holds frequency perm[p]:
+// p = q1 * M/R1 + q2 * M/(R1 R2) + ...,  k = q1 + R1 (q2 + R2 (q3 + ...))
+static void make_perm(const AxisPlan& pl, std::vector<uint16_t>& perm, std::vector<uint16_t>& inv)
+{
+    perm.assign(pl.M, 0);
+    inv.assign(pl.M, 0);
+    for (int p = 0; p < pl.M; ++p) {
+        int rem = p, span = pl.M, k = 0, w = 1;
+        for (int st = 0; st < pl.nst; ++st) {
+            span /= pl.radix[st];
+            int q = rem / span;
+            rem -= q * span;
+            k += q * w;
+            w *= pl.radix[st];
+        }
+        perm[p] = (uint16_t)k;
+        inv[k] = (uint16_t)p;
+    }
+}
+
+static bool pow2_in(int v, int lo, int hi) { return v >= lo && v <= hi && (v & (v - 1)) == 0; }
+
+extern "C" const char* fe_last_error(void) { return g_err; }
+extern "C" const char* fe_version(void) { return "fe_b200 0.1 (sm_100a)"; }
+
+static void layout_workspace(fe_grid* g)
+{
+    const Geometry& q = g->geo;
+    const int B = g->desc.batch;
+    const int Hy = q.m[1] / 2 + 1, Hz = q.m[2] / 2 + 1;
+    size_t off = 0;
+    g->o_Kt = off;  off += align_up((size_t)6 * Hz * Hy * q.pitch * g->rsz);
+    const size_t hot0 = off;
+    g->o_S1 = off;  off += align_up((size_t)B * 3 * q.n[2] * q.n[1] * q.pitch * g->csz);
+    g->o_S2 = off;  off += align_up((size_t)B * 3 * q.n[2] * q.m[1] * q.pitch * g->csz);
+    g->o_E = off;   off += align_up((size_t)B * 3 * g->N * g->rsz);
+    g->o_Y = off;   off += align_up((size_t)B * 3 * g->N * g->rsz);
+    g->o_ACC = off; off += align_up((size_t)B * 3 * g->N * g->rsz);
+    g->o_PP = off;  off += align_up((size_t)B * 3 * g->N * g->rsz);
+    const size_t hot1 = off;
+    // precompute scratch overlays the hot region (the tensor is computed before any step)
+    size_t s = hot0;
+    g->o_box = s;   s += align_up((size_t)q.m[0] * q.m[1] * q.m[2] * sizeof(double));
+    g->o_Sbox = s;  s += align_up((size_t)q.m[2] * q.m[1] * q.pitch64 * 2 * sizeof(double));
+    off = hot1 > s ? hot1 : s;
+    g->nblk = 296;
+    g->o_part = off; off += align_up((size_t)B * g->nblk * 8 * sizeof(double));
+    g->total_bytes = off;
+}
+
+extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
+{
+    if (!d || !out) return fail(FE_EINVAL, "null argument");
+    const int n[3] = {d->nx, d->ny, d->nz};
+    const double dd[3] = {d->dx, d->dy, d->dz};
+    for (int a = 0; a < 3; ++a) {
+        if (!pow2_in(n[a], 4, 1024)) return fail(FE_EINVAL, "n[%d] = %d is not a power of two in [4, 1024]", a, n[a]);
+        if (!(dd[a] > 0.0) || !isfinite(dd[a])) return fail(FE_EINVAL, "cell size d[%d] must be > 0", a);
+        if (d->periodic[a] != 0 && d->periodic[a] != 1) return fail(FE_EINVAL, "periodic[%d] must be 0 or 1", a);
+        if (d->pbc_images[a] < 0 || d->pbc_images[a] > 64) return fail(FE_EINVAL, "pbc_images[%d] out of range", a);
+    }
+    if (d->batch < 1 || d->batch > 16384) return fail(FE_EINVAL, "batch must be in [1, 16384]");
+    if (d->dtype != FE_F64 && d->dtype != FE_F32) return fail(FE_EINVAL, "dtype must be FE_F64 or FE_F32");
+    if (d->n_materials < 1 || d->n_materials > 255) return fail(FE_EINVAL, "n_materials must be in [1, 255]");
+    if ((int64_t)d->batch * 3 * d->nz > 0x7fffffffLL) return fail(FE_EINVAL, "batch * nz too large");
+
+    fe_grid* g = new (std::nothrow) fe_grid();
+    if (!g) return fail(FE_ENOMEM, "host allocation failed");
+    g->desc = *d;
+    g->f32 = d->dtype == FE_F32;
+    g->rsz = g->f32 ? 4 : 8;
+    g->csz = 2 * g->rsz;
+    g->N = (int64_t)d->nx * d->ny * d->nz;
+    Geometry& q = g->geo;
+    for (int a = 0; a < 3; ++a) {
+        q.n[a] = n[a];
+        q.periodic[a] = d->periodic[a];
+        q.images[a] = d->periodic[a] ? d->pbc_images[a] : 0;
+        q.m[a] = d->periodic[a] ? n[a] : 2 * n[a];
+        q.d[a] = dd[a];
+    }
+    q.zero_mode = d->zero_mode;
+    q.Lx = q.m[0] / 2 + 1;
+    // lanes: 128 bytes of complex numbers, halved until the fused z tile (3 components) fits in shared memory
+    auto pick_lanes = [&](size_t cxb) {
+        int l = (int)(128 / cxb);
+        while (l > 1 && zmul_smem_bytes(q.m[2], l, cxb) > 200 * 1024) l >>= 1;
+        while (l > 1 && (size_t)q.m[1] * l * cxb > 200 * 1024) l >>= 1;
+        return l;
+    };
+    q.lanes = pick_lanes(g->csz);
+    q.lanes64 = pick_lanes(16);
+    const int pl = (int)(128 / g->csz);
+    q.pitch = (q.Lx + pl - 1) / pl * pl;
+    q.pitch64 = (q.Lx + 7) / 8 * 8;
+    g->dirty = true;
+    g->mixed = 0;
+    g->map = nullptr;
+    g->ws = nullptr;
+    g->ws_bytes = 0;
+    g->tensor_ready = false;
+    g->launches = 0;
+    const int B = d->batch, M = d->n_materials;
+    g->h_mats.assign((size_t)B * M, DevLandau{});
+    g->mat_set.assign((size_t)B * M, 0);
+    g->h_members.assign(B, DevMember{});
+    g->h_globals.assign(B, fe_global{});
+    g->glob_set.assign(B, 0);
+    layout_workspace(g);
+
+    // small device tables: twiddles (fp64 + fp32), perm/invperm per axis, coefficient tables, energy out
+    AxisPlan plans[3] = {make_plan(q.m[0] / 2), make_plan(q.m[1]), make_plan(q.m[2])};
+    std::vector<uint16_t> perm[3], inv[3];
+    for (int a = 0; a < 3; ++a) make_perm(plans[a], perm[a], inv[a]);
+    size_t off = 0;
+    const size_t o_tw64 = off; off += align_up(kTwiddleN * 16);
+    const size_t o_tw32 = off; off += align_up(kTwiddleN * 8);
+    size_t o_perm[3], o_inv[3];
+    for (int a = 0; a < 3; ++a) {
+        o_perm[a] = off; off += align_up(plans[a].M * 2);
+        o_inv[a] = off;  off += align_up(plans[a].M * 2);
+    }
+    const size_t o_mats = off; off += align_up((size_t)B * M * sizeof(DevLandau));
+    const size_t o_mem = off;  off += align_up((size_t)B * sizeof(DevMember));
+    const size_t o_eout = off; off += align_up((size_t)B * 8 * sizeof(double));
+    std::vector<unsigned char> h(off, 0);
+    {
+        const long double twopi = 6.283185307179586476925286766559005768L;
+        double* t64 = reinterpret_cast<double*>(h.data() + o_tw64);
+        float* t32 = reinterpret_cast<float*>(h.data() + o_tw32);
+        for (int k = 0; k < kTwiddleN; ++k) {
+            const long double ang = twopi * k / kTwiddleN;
+            const long double c = (k == kTwiddleN / 4 || k == 3 * kTwiddleN / 4) ? 0.0L : cosl(ang);
+            const long double s = (k == 0 || k == kTwiddleN / 2) ? 0.0L : sinl(ang);
+            t64[2 * k] = (double)c;  t64[2 * k + 1] = (double)(-s);
+            t32[2 * k] = (float)c;   t32[2 * k + 1] = (float)(-s);
+        }
+        for (int a = 0; a < 3; ++a) {
+            memcpy(h.data() + o_perm[a], perm[a].data(), plans[a].M * 2);
+            memcpy(h.data() + o_inv[a], inv[a].data(), plans[a].M * 2);
+        }
+    }
+    cudaError_t e = cudaMalloc(&g->d_small, off);
+    if (e != cudaSuccess) { delete g; return fail(FE_ECUDA, "cudaMalloc(tables): %s", cudaGetErrorString(e)); }
+    e = cudaMemcpy(g->d_small, h.data(), off, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = fft_configure();
+    if (e == cudaSuccess) e = tensor_init_tables();
+    if (e != cudaSuccess) {
+        cudaFree(g->d_small);
+        delete g;
+        return fail(FE_ECUDA, "table setup: %s", cudaGetErrorString(e));
+    }
+    g->d_mats = reinterpret_cast<DevLandau*>(g->d_small + o_mats);
+    g->d_members = reinterpret_cast<DevMember*>(g->d_small + o_mem);
+    g->d_eout = reinterpret_cast<double*>(g->d_small + o_eout);
+    for (int a = 0; a < 3; ++a) {
+        g->ctx.plan[a] = g->ctx64.plan[a] = plans[a];
+        g->ctx.tab[a].perm = g->ctx64.tab[a].perm = reinterpret_cast<const uint16_t*>(g->d_small + o_perm[a]);
+        g->ctx.tab[a].invperm = g->ctx64.tab[a].invperm = reinterpret_cast<const uint16_t*>(g->d_small + o_inv[a]);
+    }
+    g->ctx64.tw = g->d_small + o_tw64;
+    g->ctx.tw = g->f32 ? g->d_small + o_tw32 : g->d_small + o_tw64;
+    *out = g;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_destroy_grid(fe_grid* g)
+{
+    if (!g) return FE_OK;
+    cudaFree(g->d_small);
+    delete g;
+    return FE_OK;
+}
+
+extern "C" size_t fe_workspace_bytes(const fe_grid* g) { return g ? g->total_bytes : 0; }
+
+extern "C" fe_status fe_padded_dims(const fe_grid* g, int32_t out[3])
+{
+    if (!g || !out) return fail(FE_EINVAL, "null argument");
+    for (int a = 0; a < 3; ++a) out[a] = g->geo.m[a];
+    return FE_OK;
+}
+
+extern "C" uint64_t fe_launch_count(const fe_grid* g) { return g ? g->launches : 0; }
+
+extern "C" fe_status fe_bind_workspace(fe_grid* g, void* dev, size_t bytes)
+{
+    if (!g || !dev) return fail(FE_EINVAL, "null argument");
+    if (bytes < g->total_bytes) return fail(FE_ENOMEM, "workspace of %zu bytes given, %zu needed", bytes, g->total_bytes);
+    if (reinterpret_cast<uintptr_t>(dev) % 256) return fail(FE_EINVAL, "workspace must be 256-byte aligned");
+    g->ws = static_cast<unsigned char*>(dev);
+    g->ws_bytes = bytes;
+    g->tensor_ready = false;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_set_material(fe_grid* g, int32_t member, int32_t id, const fe_landau* m)
+{
+    if (!g || !m) return fail(FE_EINVAL, "null argument");
+    const int B = g->desc.batch, M = g->desc.n_materials;
+    if (member < -1 || member >= B) return fail(FE_EINVAL, "member %d out of range", member);
+    if (id < 0 || id >= M) return fail(FE_EINVAL, "material id %d out of range", id);
+    const double* v = &m->a1[0];
+    for (int i = 0; i < 12; ++i)
+        if (!isfinite(v[i])) return fail(FE_EINVAL, "non-finite Landau coefficient");
+    DevLandau dl;
+    memset(&dl, 0, sizeof(dl));
+    for (int i = 0; i < 3; ++i) dl.a1[i] = m->a1[i];
+    dl.a11 = m->a11; dl.a12 = m->a12; dl.a111 = m->a111; dl.a112 = m->a112; dl.a123 = m->a123;
+    dl.a1111 = m->a1111; dl.a1112 = m->a1112; dl.a1122 = m->a1122; dl.a1123 = m->a1123;
+    dl.active = m->active ? 1 : 0;
+    for (int b = (member < 0 ? 0 : member); b < (member < 0 ? B : member + 1); ++b) {
+        g->h_mats[(size_t)b * M + id] = dl;
+        g->mat_set[(size_t)b * M + id] = 1;
+    }
+    g->dirty = true;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_set_global(fe_grid* g, int32_t member, const fe_global* gl)
+{
+    if (!g || !gl) return fail(FE_EINVAL, "null argument");
+    const int B = g->desc.batch;
+    if (member < -1 || member >= B) return fail(FE_EINVAL, "member %d out of range", member);
+    if (!(gl->eps0 > 0.0) || !(gl->epsB > 0.0) || !isfinite(gl->eps0 * gl->epsB))
+        return fail(FE_EINVAL, "eps0 and epsB must be > 0");
+    if (!isfinite(gl->G11) || !isfinite(gl->G12) || !isfinite(gl->G44) || !isfinite(gl->G44p) || !isfinite(gl->L))
+        return fail(FE_EINVAL, "non-finite coefficient");
+    for (int b = (member < 0 ? 0 : member); b < (member < 0 ? B : member + 1); ++b) {
+        DevMember& dm = g->h_members[b];
+        dm.G11 = gl->G11;
+        dm.Gt = gl->G44 + gl->G44p;
+        dm.Gm = gl->G12 + gl->G44 - gl->G44p;
+        dm.escale = 1.0 / (gl->eps0 * gl->epsB);
+        dm.L = gl->L;
+        g->h_globals[b] = *gl;
+        g->glob_set[b] = 1;
+    }
+    g->dirty = true;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_set_external_field(fe_grid* g, int32_t member, const double E[3])
+{
+    if (!g || !E) return fail(FE_EINVAL, "null argument");
+    const int B = g->desc.batch;
+    if (member < -1 || member >= B) return fail(FE_EINVAL, "member %d out of range", member);
+    for (int i = 0; i < 3; ++i)
+        if (!isfinite(E[i])) return fail(FE_EINVAL, "non-finite field");
+    for (int b = (member < 0 ? 0 : member); b < (member < 0 ? B : member + 1); ++b)
+        for (int i = 0; i < 3; ++i) g->h_members[b].Eext[i] = E[i];
+    g->dirty = true;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map)
+{
+    if (!g) return fail(FE_EINVAL, "null argument");
+    g->map = dev_map;
+    return FE_OK;
+}
+
+static fe_status sync_params(fe_grid* g, cudaStream_t st)
+{
+    const int B = g->desc.batch, M = g->desc.n_materials;
+    for (int b = 0; b < B; ++b) {
+        if (!g->glob_set[b]) return fail(FE_ESTATE, "fe_set_global was not called for member %d", b);
+        for (int m = 0; m < M; ++m)
+            if (!g->mat_set[(size_t)b * M + m]) return fail(FE_ESTATE, "material %d of member %d is unset", m, b);
+    }
+    if (!g->dirty) return FE_OK;
+    g->mixed = 0;
+    for (int b = 0; b < B; ++b)
+        if (g->h_members[b].Gm != 0.0) g->mixed = 1;
+    FE_CUDA(cudaMemcpyAsync(g->d_mats, g->h_mats.data(), (size_t)B * M * sizeof(DevLandau), cudaMemcpyHostToDevice, st));
+    FE_CUDA(cudaMemcpyAsync(g->d_members, g->h_members.data(), (size_t)B * sizeof(DevMember), cudaMemcpyHostToDevice, st));
+    // pageable host memory: the copies are staged before the calls return, the vectors may change afterwards
+    g->dirty = false;
+    return FE_OK;
+}
+
+// ---- a0 ------------------------------------------------------------------------------------------
+template <typename T>
+static fe_status precompute_T(fe_grid* g, cudaStream_t st)
+{
+    const Geometry& q = g->geo;
+    double* box = reinterpret_cast<double*>(g->ws + g->o_box);
+    void* Sbox = g->ws + g->o_Sbox;
+    T* Kt = reinterpret_cast<T*>(g->ws + g->o_Kt);
+    const int Hy = q.m[1] / 2 + 1, Hz = q.m[2] / 2 + 1;
+    const double scale = 1.0 / ((double)(q.m[0] / 2) * q.m[1] * q.m[2]);
+    const int64_t p64 = q.pitch64;
+    for (int c = 0; c < 6; ++c) {
+        FE_CUDA(launch_tensor_box(q, box, c, 1, st));
+        FE_CUDA(launch_zero_mode(q, box, c, st));
+        FE_CUDA(launch_xfwd<double>(g->ctx64, box, Sbox, q.m[0], q.m[1], q.m[2], q.m[0], (int64_t)q.m[0] * q.m[1],
+                                    p64, p64 * q.m[1], st));
+        FE_CUDA(launch_axis<double>(g->ctx64, 1, -1, Sbox, Sbox, q.m[1], q.lanes64, q.pitch64, q.m[2], 1, p64,
+                                    p64 * q.m[1], 0, p64, p64 * q.m[1], 0, st));
+        FE_CUDA(launch_axis<double>(g->ctx64, 2, -1, Sbox, Sbox, q.m[2], q.lanes64, q.pitch64, q.m[1], 1,
+                                    p64 * q.m[1], p64, 0, p64 * q.m[1], p64, 0, st));
+        FE_CUDA(launch_extract<T>(Sbox, Kt + (int64_t)c * Hz * Hy * q.pitch, q.m[2], q.m[1], q.Lx, q.pitch64, q.pitch,
+                                  scale, st));
+        g->launches += 5 + ((q.zero_mode && q.periodic[0] + q.periodic[1] + q.periodic[2] == 2) ? 1 : 0);
+    }
+    return FE_OK;
+}
+
+extern "C" fe_status fe_precompute_tensor(fe_grid* g, void* stream)
+{
+    if (!g) return fail(FE_EINVAL, "null argument");
+    if (!g->ws) return fail(FE_ESTATE, "no workspace bound");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    fe_status s = g->f32 ? precompute_T<float>(g, st) : precompute_T<double>(g, st);
+    if (s != FE_OK) return s;
+    FE_CUDA(cudaStreamSynchronize(st));
+    g->tensor_ready = true;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_get_tensor(fe_grid* g, double* host_out, void* stream)
+{
+    if (!g || !host_out) return fail(FE_EINVAL, "null argument");
+    if (!g->ws) return fail(FE_ESTATE, "no workspace bound");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const Geometry& q = g->geo;
+    // uses the spectra region as scratch: a running simulation's tensor spectrum (Kt) is untouched
+    double* box = reinterpret_cast<double*>(g->ws + g->o_box);
+    const int64_t total = (int64_t)q.m[0] * q.m[1] * q.m[2];
+    for (int c = 0; c < 6; ++c) {
+        FE_CUDA(launch_tensor_box(q, box, c, 1, st));
+        FE_CUDA(launch_zero_mode(q, box, c, st));
+        FE_CUDA(cudaMemcpyAsync(host_out + c * total, box, total * sizeof(double), cudaMemcpyDeviceToHost, st));
+        FE_CUDA(cudaStreamSynchronize(st));
+        g->launches += 2;
+    }
+    return FE_OK;
+}
+
+// ---- a1-a3: electrostatic field of state Y into the E buffer ------------------------------------------
+template <typename T>
+static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
+{
+    const Geometry& q = g->geo;
+    const int B = g->desc.batch;
+    void* S1 = g->ws + g->o_S1;
+    void* S2 = g->ws + g->o_S2;
+    T* E = reinterpret_cast<T*>(g->ws + g->o_E);
+    const T* Kt = reinterpret_cast<const T*>(g->ws + g->o_Kt);
+    const int64_t p = q.pitch;
+    const int slabs = B * 3 * q.n[2];
+    FE_CUDA(launch_xfwd<T>(g->ctx, Y, S1, q.n[0], q.n[1], slabs, q.n[0], (int64_t)q.n[0] * q.n[1], p, p * q.n[1], st));
+    FE_CUDA(launch_axis<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.n[1],
+                           p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
+    FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
+    FE_CUDA(launch_axis<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.m[1],
+                           p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
+    FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
+    g->launches += 5;
+    return FE_OK;
+}
+
+template <typename T>
+static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double cy, const T* accIn, T* accOut, double ca,
+                       uint32_t terms, cudaStream_t st)
+{
+    const bool elec = (terms & FE_TERM_ELEC) != 0;
+    if (elec) {
+        fe_status s = elec_field<T>(g, Y, st);
+        if (s != FE_OK) return s;
+    }
+    LocalArgs a;
+    memset(&a, 0, sizeof(a));
+    a.Y = Y;
+    a.Eelec = elec ? g->ws + g->o_E : nullptr;
+    a.baseY = baseY;
+    a.Yout = Yout;
+    a.accIn = accIn;
+    a.accOut = accOut;
+    a.cy = cy;
+    a.ca = ca;
+    a.map = g->map;
+    a.mats = g->d_mats;
+    a.members = g->d_members;
+    a.nmat = g->desc.n_materials;
+    for (int i = 0; i < 3; ++i) { a.n[i] = g->geo.n[i]; a.periodic[i] = g->geo.periodic[i]; a.d[i] = g->geo.d[i]; }
+    a.terms = terms;
+    a.batch = g->desc.batch;
+    a.mixed = g->mixed;
+    FE_CUDA(launch_local<T>(a, st));
+    g->launches += 1;
+    return FE_OK;
+}
+
+static fe_status check_ready(fe_grid* g, const void* P, uint32_t terms)
+{
+    if (!g || !P) return fail(FE_EINVAL, "null argument");
+    if (terms & ~(uint32_t)FE_TERM_ALL) return fail(FE_EINVAL, "unknown bits in terms");
+    if (reinterpret_cast<uintptr_t>(P) % 16) return fail(FE_EINVAL, "state arrays must be 16-byte aligned");
+    if (!g->ws) return fail(FE_ESTATE, "no workspace bound");
+    if ((terms & FE_TERM_ELEC) && !g->tensor_ready)
+        return fail(FE_ESTATE, "FE_TERM_ELEC requested before fe_precompute_tensor");
+    return FE_OK;
+}
+
+extern "C" fe_status fe_rhs(fe_grid* g, const void* P, void* dPdt, uint32_t terms, void* stream)
+{
+    fe_status s = check_ready(g, P, terms);
+    if (s != FE_OK) return s;
+    if (!dPdt || dPdt == P) return fail(FE_EINVAL, "dPdt must be a distinct array");
+    if (reinterpret_cast<uintptr_t>(dPdt) % 16) return fail(FE_EINVAL, "state arrays must be 16-byte aligned");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((s = sync_params(g, st)) != FE_OK) return s;
+    if (g->f32) return stage<float>(g, (const float*)P, nullptr, (float*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st);
+    return stage<double>(g, (const double*)P, nullptr, (double*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st);
+}
+
+template <typename T>
+static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint32_t terms, cudaStream_t st)
+{
+    T* Y = reinterpret_cast<T*>(g->ws + g->o_Y);
+    T* ACC = reinterpret_cast<T*>(g->ws + g->o_ACC);
+    T* PP = reinterpret_cast<T*>(g->ws + g->o_PP);
+    const size_t bytes = (size_t)g->desc.batch * 3 * g->N * sizeof(T);
+    fe_status s;
+    if (integ == FE_EULER) {
+        T* cur = P;
+        T* nxt = PP;
+        for (int i = 0; i < nsteps; ++i) {
+            if ((s = stage<T>(g, cur, cur, nxt, dt, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+            T* t = cur; cur = nxt; nxt = t;
+        }
+        if (cur != P) FE_CUDA(cudaMemcpyAsync(P, cur, bytes, cudaMemcpyDeviceToDevice, st));
+    } else if (integ == FE_HEUN) {
+        for (int i = 0; i < nsteps; ++i) {
+            // k1 = f(P): Y = P + dt k1, ACC = P + dt/2 k1;  k2 = f(Y): P = ACC + dt/2 k2
+            if ((s = stage<T>(g, P, P, Y, dt, P, ACC, 0.5 * dt, terms, st)) != FE_OK) return s;
+            if ((s = stage<T>(g, Y, ACC, P, 0.5 * dt, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+        }
+    } else {
+        for (int i = 0; i < nsteps; ++i) {
+            // classical RK4, weights 1/6 1/3 1/3 1/6, stage points P + dt/2 k1, P + dt/2 k2, P + dt k3
+            if ((s = stage<T>(g, P, P, Y, 0.5 * dt, P, ACC, dt / 6.0, terms, st)) != FE_OK) return s;
+            if ((s = stage<T>(g, Y, P, PP, 0.5 * dt, ACC, ACC, dt / 3.0, terms, st)) != FE_OK) return s;
+            if ((s = stage<T>(g, PP, P, Y, dt, ACC, ACC, dt / 3.0, terms, st)) != FE_OK) return s;
+            if ((s = stage<T>(g, Y, ACC, P, dt / 6.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+        }
+    }
+    return FE_OK;
+}
+
+extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int32_t integ, uint32_t terms, void* stream)
+{
+    fe_status s = check_ready(g, P, terms);
+    if (s != FE_OK) return s;
+    if (nsteps < 0) return fail(FE_EINVAL, "nsteps < 0");
+    if (!isfinite(dt)) return fail(FE_EINVAL, "dt not finite");
+    if (integ != FE_EULER && integ != FE_HEUN && integ != FE_RK4) return fail(FE_EINVAL, "unknown integrator");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((s = sync_params(g, st)) != FE_OK) return s;
+    if (g->f32) return step_T<float>(g, (float*)P, dt, nsteps, integ, terms, st);
+    return step_T<double>(g, (double*)P, dt, nsteps, integ, terms, st);
+}
+
+extern "C" fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double* host_out, void* stream)
+{
+    fe_status s = check_ready(g, P, terms);
+    if (s != FE_OK) return s;
+    if (!host_out) return fail(FE_EINVAL, "null argument");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((s = sync_params(g, st)) != FE_OK) return s;
+    const bool elec = (terms & FE_TERM_ELEC) != 0;
+    if (elec) {
+        s = g->f32 ? elec_field<float>(g, (const float*)P, st) : elec_field<double>(g, (const double*)P, st);
+        if (s != FE_OK) return s;
+    }
+    EnergyArgs a;
+    memset(&a, 0, sizeof(a));
+    a.P = P;
+    a.Eelec = elec ? g->ws + g->o_E : nullptr;
+    a.map = g->map;
+    a.mats = g->d_mats;
+    a.members = g->d_members;
+    a.nmat = g->desc.n_materials;
+    for (int i = 0; i < 3; ++i) { a.n[i] = g->geo.n[i]; a.periodic[i] = g->geo.periodic[i]; a.d[i] = g->geo.d[i]; }
+    a.terms = terms;
+    a.batch = g->desc.batch;
+    a.partials = reinterpret_cast<double*>(g->ws + g->o_part);
+    a.out = g->d_eout;
+    a.nblk = g->nblk;
+    FE_CUDA(g->f32 ? launch_energy<float>(a, st) : launch_energy<double>(a, st));
+    g->launches += 2;
+    const size_t nb = (size_t)g->desc.batch * 8;
+    FE_CUDA(cudaMemcpyAsync(host_out, g->d_eout, nb * sizeof(double), cudaMemcpyDeviceToHost, st));
+    FE_CUDA(cudaStreamSynchronize(st));
+    for (size_t i = 0; i < nb; ++i)
+        if (!isfinite(host_out[i])) return fail(FE_ENONFINITE, "non-finite energy or mean (entry %zu)", i);
+    return FE_OK;
+}

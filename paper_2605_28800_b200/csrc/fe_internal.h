@@ -1,0 +1,141 @@
+// fe_internal.h -- host-side declarations shared by the translation units of libfe_b200.
+// Not part of the ABI (include/fe.h is).  No code here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+namespace fe {
+
+constexpr int kTwiddleN = 2048;      // twiddle table w[k] = exp(-2 pi i k / 2048); covers every axis length
+constexpr int kMaxStages = 6;
+constexpr int kThreads = 256;
+
+// Radix plan of one in-place power-of-two FFT of length M (complex points).
+// Forward = decimation in frequency (natural in, digit-reversed out),
+// inverse = decimation in time with the stages mirrored (digit-reversed in, natural out).
+struct AxisPlan {
+    int M;                  // transform length
+    int logM;
+    int nst;                // number of stages
+    int radix[kMaxStages];  // product = M, each in {8, 4, 2}
+};
+
+// device-resident index tables of one axis
+struct AxisTables {
+    const uint16_t* perm;     // position p after the forward stages holds frequency perm[p]
+    const uint16_t* invperm;  // frequency k sits at position invperm[k]
+};
+
+// Per-member scalars as the kernels read them.
+struct DevMember {
+    double G11, Gt, Gm;      // Gt = G44 + G44', Gm = G12 + G44 - G44' (Eq. 4 expanded, O2)
+    double escale;           // 1 / (eps0 * epsB)   (Eq. 6 prefactor)
+    double L;
+    double Eext[3];
+};
+
+struct DevLandau {
+    double a1[3];
+    double a11, a12, a111, a112, a123;
+    double a1111, a1112, a1122, a1123;
+    int32_t active;
+    int32_t pad;
+};
+
+struct Geometry {
+    int n[3];          // nx ny nz
+    int m[3];          // padded box
+    int periodic[3];
+    int images[3];
+    double d[3];
+    int zero_mode;
+    int Lx;            // m[0]/2 + 1 complex points per spectrum row
+    int pitch;         // row pitch of the spectra (complex elements), multiple of the lane tile
+    int pitch64;       // same for the fp64 precompute spectra
+    int lanes;         // kx lanes per block in the strided passes (128 B of complex numbers)
+    int lanes64;
+};
+
+// ---- launchers (fe_fft.cu) --------------------------------------------------------------------
+struct FftCtx {
+    const void* tw;           // cx<T>[kTwiddleN]
+    AxisPlan plan[3];         // [0]: x (length m_x/2 complex), [1]: y, [2]: z
+    AxisTables tab[3];
+};
+
+// real rows -> half spectrum rows.  in: T real rows of n_in valid reals (zero-padded to 2*plan.M),
+// out: complex rows of pitch `pitch` holding plan.M + 1 entries.
+template <typename T>
+cudaError_t launch_xfwd(const FftCtx& c, const T* in, void* out, int n_in, int rows_per_slab, int slabs,
+                        int64_t in_row_stride, int64_t in_slab_stride, int64_t out_row_stride,
+                        int64_t out_slab_stride, cudaStream_t st);
+template <typename T>
+cudaError_t launch_xinv(const FftCtx& c, const void* in, T* out, int n_out, int rows_per_slab, int slabs,
+                        int64_t in_row_stride, int64_t in_slab_stride, int64_t out_row_stride,
+                        int64_t out_slab_stride, cudaStream_t st);
+// strided pass along one axis (axis = 1 or 2 picks plan/tables): forward reads n_keep rows and writes
+// plan.M rows (natural frequency order); inverse reads plan.M rows and writes n_keep rows.
+template <typename T>
+cudaError_t launch_axis(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep,
+                        int lanes, int pitch_used, int outer, int batch, int64_t in_sa, int64_t in_so,
+                        int64_t in_sb, int64_t out_sa, int64_t out_so, int64_t out_sb, cudaStream_t st);
+// fused z-forward, K multiply, z-inverse, in place on S[b][3][nz][My][pitch]
+template <typename T>
+cudaError_t launch_zmul(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My,
+                        int lanes, int pitch, int batch, cudaStream_t st);
+// complex fp64 box spectrum -> real octant table of T (scaled)
+template <typename T>
+cudaError_t launch_extract(const void* Sbox, T* Kt_comp, int Mz, int My, int Lx, int pitch64, int pitchT,
+                           double scale, cudaStream_t st);
+size_t zmul_smem_bytes(int Mz, int lanes, size_t cx_bytes);
+cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
+
+// ---- tensor (fe_tensor.cu) --------------------------------------------------------------------
+cudaError_t tensor_init_tables();
+// real-space kernel of one component on the circular box [mz][my][mx] (fp64)
+cudaError_t launch_tensor_box(const Geometry& g, double* box6 /* [6][mz][my][mx] or one comp */,
+                              int comp_first, int ncomp, cudaStream_t st);
+cudaError_t launch_zero_mode(const Geometry& g, double* box, int comp, cudaStream_t st);
+
+// ---- local terms (fe_local.cu) ----------------------------------------------------------------
+struct LocalArgs {
+    const void* Y;        // state the RHS is evaluated at           [B][3][N]
+    const void* Eelec;    // electrostatic field (may be null)       [B][3][N]
+    const void* baseY;    // Yout = baseY + cy * k  (null: Yout = cy * k)
+    void* Yout;
+    const void* accIn;    // accOut = accIn + ca * k (both null: skipped)
+    void* accOut;
+    double cy, ca;
+    const uint8_t* map;   // null: material 0 everywhere
+    const DevLandau* mats;    // [B][nmat]
+    const DevMember* members; // [B]
+    int nmat;
+    int n[3];
+    int periodic[3];
+    double d[3];
+    uint32_t terms;
+    int batch;
+    int mixed;            // any member has Gm != 0
+};
+template <typename T> cudaError_t launch_local(const LocalArgs& a, cudaStream_t st);
+
+struct EnergyArgs {
+    const void* P;
+    const void* Eelec;
+    const uint8_t* map;
+    const DevLandau* mats;
+    const DevMember* members;
+    int nmat;
+    int n[3];
+    int periodic[3];
+    double d[3];
+    uint32_t terms;
+    int batch;
+    double* partials;     // [B][nblk][8]
+    double* out;          // [B][8] device
+    int nblk;
+};
+template <typename T> cudaError_t launch_energy(const EnergyArgs& a, cudaStream_t st);
+
+}  // namespace fe
