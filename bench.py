@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- TDGL cell-updates/s of the hand-written sm_100a hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5a|cfg5b|cfg3|cfg1] [--dtype f64|f32]
+    python bench.py --impl reference ...      # the CPU oracle on a bounded sample (rank 0 only)
+
+A step = one forward-Euler step of the whole hot path (pruned x/y transforms, fused z
+transform + tensor multiply, inverse transforms, fused local step) over the synthetic workload.  One JSON line
+is printed by rank 0.  N > 1: every rank runs an independent replica of the workload (batch sharding, no
+data-path collective), value = all ranks' cell-updates / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import fe_inputs as fi  # noqa: E402
+
+METRIC = "TDGL cell-updates/s (fp64, incl. FFT electrostatics)"
+UNIT = "cell-updates/s"
+
+
+def make_workload(name: str, dtype: str) -> fi.Workload:
+    if name == "cfg5a":
+        return fi.config5a(dtype)
+    if name == "cfg5b":
+        return fi.config5b(dtype)
+    if name == "cfg3":
+        w = fi.config3()
+        w.dtype = dtype
+        return w
+    if name == "cfg1":
+        w = fi.config1()
+        w.dtype = dtype
+        return w
+    raise SystemExit("unknown workload " + name)
+
+
+def sample_workload(name: str) -> fi.Workload:
+    """Bounded sample of the benchmark workload for the CPU oracle: same recipe (BaTiO3 300 K, 1 nm cells, open
+    boundaries, |P| = 0.26 sphere-uniform, Euler dt* = 0.002), 64x64x32 cells instead of 256x256x128."""
+    if name == "cfg1":
+        return fi.config1()
+    return fi.open_batio3("sample_64x64x32", (64, 64, 32), 1, "f64", 1005)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return json.load(fh), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+def algorithmic_bytes(w: fi.Workload, rsz: int):
+    """Algorithmic bytes per launch of each kernel: what the pass must read and
+    write once, spectra counted with Lx = m_x/2 + 1 columns."""
+    nx, ny, nz = w.n
+    m = [w.n[a] if w.periodic[a] else 2 * w.n[a] for a in range(3)]
+    Lx, B, c = m[0] // 2 + 1, w.batch, 2 * rsz
+    N = nx * ny * nz
+    return {
+        "xfwd": B * 3 * (N * rsz + nz * ny * Lx * c),
+        "yfwd": B * 3 * (nz * ny * Lx * c + nz * m[1] * Lx * c),
+        "zmul": B * 3 * 2 * nz * m[1] * Lx * c + 6 * (m[2] // 2 + 1) * (m[1] // 2 + 1) * Lx * rsz,
+        "yinv": B * 3 * (nz * ny * Lx * c + nz * m[1] * Lx * c),
+        "xinv": B * 3 * (N * rsz + nz * ny * Lx * c),
+        "local": B * 3 * N * rsz * 3,          # read P, read E_elec, write P_new
+    }
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2605_28800_b200 as fe
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    fe.load()
+
+    w = make_workload(args.workload, args.dtype)
+    rsz = 8 if args.dtype == "f64" else 4
+    g = fe.Grid.from_workload(w, device=dev, dtype=args.dtype)
+    t0 = time.time()
+    g.precompute_tensor()
+    t_pre = time.time() - t0
+    P_host = torch.from_numpy(w.P0.astype(np.float64 if args.dtype == "f64" else np.float32)).pin_memory()
+    P = P_host.to(dev, non_blocking=False).contiguous()
+    cells = w.cells * w.batch
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps in one fe_step call -------------
+    g.step(P, w.dt, args.warmup, fe.FE_EULER, fe.FE_TERM_ALL)
+    barrier()
+    l0 = g.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as cs:
+        ev0.record()
+        g.step(P, w.dt, args.steps, fe.FE_EULER, fe.FE_TERM_ALL)
+        ev1.record()
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = g.launch_count() - l0
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = cells * world * args.steps / (ms * 1e-3)
+    en = g.energy(P)[0]
+
+    # ---- per-kernel durations, measured live with CUDA events on the launching stream (second pass of K steps)
+    g.profile(True)
+    g.step(P, w.dt, args.steps, fe.FE_EULER, fe.FE_TERM_ALL)
+    prof = g.profile_read()
+    g.profile(False)
+    alg = algorithmic_bytes(w, rsz)
+    pk, pk_kind = peaks()
+    kern = {}
+    for k, (tms, cnt) in prof.items():
+        if cnt and k in alg:
+            dur = tms / cnt
+            kern[k] = {"ms": dur, "alg_gbs": alg[k] / (dur * 1e-3) / 1e9, "launches": cnt}
+    prof_total = sum(v["ms"] for v in kern.values())
+    dom = max(kern, key=lambda k: kern[k]["ms"])
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")     # bytes per launch from the committed ncu capture
+    if os.path.exists(tp):
+        with open(tp) as fh:
+            traffic = json.load(fh).get("%s_%s" % (args.workload, args.dtype), {}).get(dom)
+    roofline = {"bound": "hbm", "kernel": "k_" + dom, "achieved": kern[dom]["alg_gbs"], "peak": pk["hbm_gbs"],
+                "peak_kind": pk_kind + " (burst copy bandwidth, MEASURED_PEAKS.json)", "unit": "GB/s",
+                "frac": kern[dom]["alg_gbs"] / pk["hbm_gbs"], "traffic": traffic,
+                "share_of_step": kern[dom]["ms"] / prof_total,
+                "whole_step": {"alg_bytes_per_cell": sum(alg.values()) / cells,
+                               "achieved": sum(alg.values()) / (ms / args.steps * 1e-3) / 1e9,
+                               "frac": sum(alg.values()) / (ms / args.steps * 1e-3) / 1e9 / pk["hbm_gbs"]},
+                "kernels": kern}
+
+    # ---- end to end through the C ABI with host buffers: H2D of the state, one step, D2H of the result ----
+    out_host = torch.empty_like(P_host)
+    e2e_steps = max(1, min(args.steps, 5))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        P.copy_(P_host, non_blocking=True)
+        g.step(P, w.dt, 1, fe.FE_EULER, fe.FE_TERM_ALL)
+        out_host.copy_(P, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    nbytes = P_host.numel() * P_host.element_size()
+    e2e = {"value": cells * world * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+           "d2h_bytes_per_step": nbytes, "steps": e2e_steps}
+
+    # ---- cuFFT comparison (timed baseline, not the product): unpruned pad + rfftn + multiply + irfftn + crop
+    cufft = None
+    if rank == 0 and not args.no_cufft:
+        try:
+            cufft = cufft_pipeline_ms(torch, w, args.dtype, dev)
+            ours = sum(kern[k]["ms"] for k in ("xfwd", "yfwd", "zmul", "yinv", "xinv") if k in kern)
+            cufft["ours_ms"] = ours
+            cufft["speedup"] = cufft["ms"] / ours
+        except Exception as exc:      # out of memory on small boxes etc.: report, do not fail the bench
+            cufft = {"error": str(exc)[:200]}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(args.workload)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+                "config": {"workload": w.name, "grid": list(w.n), "batch": w.batch, "integrator": "euler",
+                           "terms": "landau+gradient+elec+ext", "padded_fft": [2 * v for v in w.n],
+                           "l2": "state and spectra exceed L2 (P 3N reals, spectra >= 4x that)",
+                           "parallelism": "replicas x%d" % world},
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "clocks": cs.summary(), "cufft_baseline": cufft, "precompute_s": t_pre,
+                "energy_after": {"F_tot": float(en[4]), "finite": bool(np.isfinite(en).all())}}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cufft_pipeline_ms(torch, w, dtype, dev):
+    """torch.fft (cuFFT) on the zero-padded box + an elementwise 6-component multiply, same sizes."""
+    td = torch.float64 if dtype == "f64" else torch.float32
+    nx, ny, nz = w.n
+    m = [w.n[a] if w.periodic[a] else 2 * w.n[a] for a in range(3)]
+    B = w.batch
+    P = torch.randn(B, 3, nz, ny, nx, device=dev, dtype=td)
+    K = [torch.randn(m[2], m[1], m[0] // 2 + 1, device=dev, dtype=td) for _ in range(6)]
+    idx = ((0, 3, 4), (3, 1, 5), (4, 5, 2))
+
+    def once():
+        Pp = torch.zeros(B, 3, m[2], m[1], m[0], device=dev, dtype=td)
+        Pp[:, :, :nz, :ny, :nx] = P
+        Ph = torch.fft.rfftn(Pp, dim=(2, 3, 4))
+        del Pp
+        Eh = torch.stack([sum(K[idx[i][j]] * Ph[:, j] for j in range(3)) for i in range(3)], dim=1)
+        del Ph
+        return torch.fft.irfftn(Eh, s=(m[2], m[1], m[0]), dim=(2, 3, 4))[:, :, :nz, :ny, :nx].contiguous()
+
+    for _ in range(2):
+        once()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 3
+    e0.record()
+    for _ in range(reps):
+        once()
+    e1.record()
+    torch.cuda.synchronize()
+    return {"ms": e0.elapsed_time(e1) / reps, "what": "torch.fft.rfftn/irfftn (cuFFT) on the padded box + multiply"}
+
+
+# ---------------------------------------------------------------------------------------------------------
+def oracle_steps(workload: str, steps: int, warmup: int):
+    """Time the CPU oracle as it stands (oracle-FFT electrostatics O8 + Landau + gradient + Euler) on the sample."""
+    from oracle import fe_oracle as orc
+    w = sample_workload(workload)
+    p = orc.Problem(n=w.n, d=w.d, periodic=w.periodic, pbc_images=w.pbc_images, materials=w.materials[0],
+                    g=w.globals_[0], matmap=w.matmap)
+    o = orc.Oracle(p, elec="fft")
+    o.table()                                  # tensor table: once per geometry, outside the timed region
+    P = w.P0[0].copy()
+    for _ in range(warmup):
+        P = o.step(P, w.dt, 1, fi.EULER, fi.TERM_ALL)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        P = o.step(P, w.dt, 1, fi.EULER, fi.TERM_ALL)
+    dt = time.perf_counter() - t0
+    return w, dt
+
+
+def cpu_baseline(workload: str):
+    w, dt = oracle_steps(workload, 3, 1)
+    return {"value": w.cells * 3 / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%s: %dx%dx%d cells of the same recipe, 3 Euler steps, oracle-FFT electrostatics (numpy.fft) + "
+                      "C loops for Landau/gradient, single thread; tensor table built outside the timed region"
+                      % (w.name, *w.n), "host_cores": os.cpu_count()}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps, warm = args.steps, min(args.warmup, 1)
+    steps = min(steps, 10)
+    w, dt = oracle_steps(args.workload, steps, warm)
+    value = w.cells * steps / dt
+    sample = "%s (%dx%dx%d cells, same recipe as %s), %d Euler steps" % (w.name, *w.n, args.workload, steps)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+            "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": make_workload_name(args.workload), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def make_workload_name(name: str) -> str:
+    return {"cfg5a": "cfg5a_256x256x128", "cfg5b": "cfg5b_128x128x64_b4", "cfg3": "cfg3_sweep_64^3_b16",
+            "cfg1": "cfg1_tiny_16x16x8"}[name]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg5a", choices=["cfg5a", "cfg5b", "cfg3", "cfg1"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -118,6 +118,14 @@ fe_status fe_padded_dims(const fe_grid* g, int32_t out[3]);
 /* number of kernel launches issued by this grid since creation (bench.py's gpu_launches claim) */
 uint64_t  fe_launch_count(const fe_grid* g);
 
+/* Per-kernel timing for the roofline report: while enabled, fe_rhs/fe_step record a CUDA event on the
+ * stream before every kernel launch.  fe_profile_read synchronises the stream and returns, per kernel
+ * kind {0 x-forward, 1 y-forward, 2 fused z + tensor multiply, 3 y-inverse, 4 x-inverse, 5 local step,
+ * 6 other}, the summed device time in ms (host_ms[7]) and the launch count (host_counts[7]) since the last
+ * read, then clears the record. */
+fe_status fe_profile(fe_grid* g, int32_t enable);
+fe_status fe_profile_read(fe_grid* g, double* host_ms, uint64_t* host_counts, void* cuda_stream);
+
 const char* fe_last_error(void);
 const char* fe_version(void);
 

@@ -23,7 +23,8 @@ FE_EULER, FE_HEUN, FE_RK4 = 0, 1, 2
 SYMBOLS = ["fe_create_grid", "fe_destroy_grid", "fe_workspace_bytes", "fe_bind_workspace", "fe_set_material",
            "fe_set_global", "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs",
            "fe_step", "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_launch_count", "fe_last_error",
-           "fe_version"]
+           "fe_version", "fe_profile", "fe_profile_read"]
+KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other"]
 
 
 class fe_grid_desc(ctypes.Structure):
@@ -81,13 +82,15 @@ def load():
         L.fe_energy.argtypes = [vp, vp, u32, ctypes.POINTER(dbl), vp]
         L.fe_get_tensor.argtypes = [vp, ctypes.POINTER(dbl), vp]
         L.fe_padded_dims.argtypes = [vp, ctypes.POINTER(i32)]
+        L.fe_profile.argtypes = [vp, i32]
+        L.fe_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_uint64), vp]
         L.fe_launch_count.argtypes = [vp]
         L.fe_launch_count.restype = ctypes.c_uint64
         L.fe_last_error.restype = ctypes.c_char_p
         L.fe_version.restype = ctypes.c_char_p
         for name in ("fe_create_grid", "fe_destroy_grid", "fe_bind_workspace", "fe_set_material", "fe_set_global",
                      "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs", "fe_step",
-                     "fe_energy", "fe_get_tensor", "fe_padded_dims"):
+                     "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_profile", "fe_profile_read"):
             getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -190,6 +193,18 @@ def fe_get_tensor(h) -> np.ndarray:
     return out
 
 
+def fe_profile(h, enable: bool):
+    _check(load().fe_profile(h, int(bool(enable))))
+
+
+def fe_profile_read(h):
+    """{kind: (total ms, launches)} since the last read."""
+    ms = (ctypes.c_double * 7)()
+    cnt = (ctypes.c_uint64 * 7)()
+    _check(load().fe_profile_read(h, ms, cnt, _stream()))
+    return {k: (ms[i], int(cnt[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
 def fe_launch_count(h) -> int:
     return int(load().fe_launch_count(h))
 
@@ -256,6 +271,8 @@ class Grid:
 
     def get_tensor(self) -> np.ndarray: return fe_get_tensor(self.h)
     def launch_count(self) -> int: return fe_launch_count(self.h)
+    def profile(self, enable: bool): fe_profile(self.h, enable)
+    def profile_read(self): return fe_profile_read(self.h)
 
     def close(self):
         if self.h is not None:

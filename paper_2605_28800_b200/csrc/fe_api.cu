@@ -61,7 +61,30 @@ struct fe_grid {
     int nblk;
     bool tensor_ready;
     uint64_t launches;
+    // optional per-kernel CUDA-event timing (fe_profile): event i precedes the launch of kind prof_kind[i]
+    bool prof_on;
+    std::vector<cudaEvent_t> prof_ev;
+    std::vector<int> prof_kind;
+    size_t prof_used;
 };
+
+enum { K_XFWD = 0, K_YFWD, K_ZMUL, K_YINV, K_XINV, K_LOCAL, K_OTHER, K_NKINDS };
+
+// record an event on the stream before a launch of `kind` (kind < 0: closes the previous interval)
+static void mark(fe_grid* g, int kind, cudaStream_t st)
+{
+    if (!g->prof_on) return;
+    if (g->prof_used >= 60000) return;
+    if (g->prof_used == g->prof_ev.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        g->prof_ev.push_back(e);
+        g->prof_kind.push_back(-1);
+    }
+    cudaEventRecord(g->prof_ev[g->prof_used], st);
+    g->prof_kind[g->prof_used] = kind;
+    ++g->prof_used;
+}
 
 static AxisPlan make_plan(int M)
 {
@@ -187,6 +210,8 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     g->ws_bytes = 0;
     g->tensor_ready = false;
     g->launches = 0;
+    g->prof_on = false;
+    g->prof_used = 0;
     const int B = d->batch, M = d->n_materials;
     g->h_mats.assign((size_t)B * M, DevLandau{});
     g->mat_set.assign((size_t)B * M, 0);
@@ -254,6 +279,7 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
 extern "C" fe_status fe_destroy_grid(fe_grid* g)
 {
     if (!g) return FE_OK;
+    for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
     cudaFree(g->d_small);
     delete g;
     return FE_OK;
@@ -436,12 +462,17 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     const T* Kt = reinterpret_cast<const T*>(g->ws + g->o_Kt);
     const int64_t p = q.pitch;
     const int slabs = B * 3 * q.n[2];
+    mark(g, K_XFWD, st);
     FE_CUDA(launch_xfwd<T>(g->ctx, Y, S1, q.n[0], q.n[1], slabs, q.n[0], (int64_t)q.n[0] * q.n[1], p, p * q.n[1], st));
+    mark(g, K_YFWD, st);
     FE_CUDA(launch_axis<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.n[1],
                            p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
+    mark(g, K_ZMUL, st);
     FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
+    mark(g, K_YINV, st);
     FE_CUDA(launch_axis<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.m[1],
                            p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
+    mark(g, K_XINV, st);
     FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
     g->launches += 5;
     return FE_OK;
@@ -474,6 +505,7 @@ static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double c
     a.terms = terms;
     a.batch = g->desc.batch;
     a.mixed = g->mixed;
+    mark(g, K_LOCAL, st);
     FE_CUDA(launch_local<T>(a, st));
     g->launches += 1;
     return FE_OK;
@@ -498,8 +530,10 @@ extern "C" fe_status fe_rhs(fe_grid* g, const void* P, void* dPdt, uint32_t term
     if (reinterpret_cast<uintptr_t>(dPdt) % 16) return fail(FE_EINVAL, "state arrays must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = sync_params(g, st)) != FE_OK) return s;
-    if (g->f32) return stage<float>(g, (const float*)P, nullptr, (float*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st);
-    return stage<double>(g, (const double*)P, nullptr, (double*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st);
+    s = g->f32 ? stage<float>(g, (const float*)P, nullptr, (float*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st)
+               : stage<double>(g, (const double*)P, nullptr, (double*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st);
+    mark(g, -1, st);
+    return s;
 }
 
 template <typename T>
@@ -517,7 +551,10 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
             if ((s = stage<T>(g, cur, cur, nxt, dt, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
             T* t = cur; cur = nxt; nxt = t;
         }
-        if (cur != P) FE_CUDA(cudaMemcpyAsync(P, cur, bytes, cudaMemcpyDeviceToDevice, st));
+        if (cur != P) {
+            mark(g, K_OTHER, st);
+            FE_CUDA(cudaMemcpyAsync(P, cur, bytes, cudaMemcpyDeviceToDevice, st));
+        }
     } else if (integ == FE_HEUN) {
         for (int i = 0; i < nsteps; ++i) {
             // k1 = f(P): Y = P + dt k1, ACC = P + dt/2 k1;  k2 = f(Y): P = ACC + dt/2 k2
@@ -545,8 +582,10 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
     if (integ != FE_EULER && integ != FE_HEUN && integ != FE_RK4) return fail(FE_EINVAL, "unknown integrator");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = sync_params(g, st)) != FE_OK) return s;
-    if (g->f32) return step_T<float>(g, (float*)P, dt, nsteps, integ, terms, st);
-    return step_T<double>(g, (double*)P, dt, nsteps, integ, terms, st);
+    s = g->f32 ? step_T<float>(g, (float*)P, dt, nsteps, integ, terms, st)
+               : step_T<double>(g, (double*)P, dt, nsteps, integ, terms, st);
+    mark(g, -1, st);
+    return s;
 }
 
 extern "C" fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double* host_out, void* stream)
@@ -582,5 +621,31 @@ extern "C" fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double
     FE_CUDA(cudaStreamSynchronize(st));
     for (size_t i = 0; i < nb; ++i)
         if (!isfinite(host_out[i])) return fail(FE_ENONFINITE, "non-finite energy or mean (entry %zu)", i);
+    return FE_OK;
+}
+
+// ---- per-kernel timing (bench.py's roofline leg) ------------------------------------------------------
+extern "C" fe_status fe_profile(fe_grid* g, int32_t enable)
+{
+    if (!g) return fail(FE_EINVAL, "null argument");
+    g->prof_on = enable != 0;
+    g->prof_used = 0;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_profile_read(fe_grid* g, double* host_ms, uint64_t* host_counts, void* stream)
+{
+    if (!g || !host_ms || !host_counts) return fail(FE_EINVAL, "null argument");
+    FE_CUDA(cudaStreamSynchronize(static_cast<cudaStream_t>(stream)));
+    for (int k = 0; k < K_NKINDS; ++k) { host_ms[k] = 0.0; host_counts[k] = 0; }
+    for (size_t i = 0; i + 1 < g->prof_used; ++i) {
+        const int kind = g->prof_kind[i];
+        if (kind < 0) continue;
+        float ms = 0.f;
+        FE_CUDA(cudaEventElapsedTime(&ms, g->prof_ev[i], g->prof_ev[i + 1]));
+        host_ms[kind] += ms;
+        host_counts[kind] += 1;
+    }
+    g->prof_used = 0;
     return FE_OK;
 }
