@@ -7,6 +7,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <new>
 #include <vector>
@@ -60,6 +61,7 @@ struct fe_grid {
     size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_part, o_box, o_Sbox, total_bytes;
     int nblk;
     bool tensor_ready;
+    bool fast[3];                    // size-specialised register FFT kernels available for the x / y / z pass
     uint64_t launches;
     // optional per-kernel CUDA-event timing (fe_profile): event i precedes the launch of kind prof_kind[i]
     bool prof_on;
@@ -203,6 +205,15 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     const int pl = (int)(128 / g->csz);
     q.pitch = (q.Lx + pl - 1) / pl * pl;
     q.pitch64 = (q.Lx + 7) / 8 * 8;
+    {
+        // FE_B200_GENERIC=1 forces the generic shared-memory passes (debugging aid; both paths are tested)
+        const char* env = getenv("FE_B200_GENERIC");
+        const bool generic = env && env[0] == '1';
+        const size_t lanes_full = 128 / g->csz;
+        g->fast[0] = !generic && x2_supported(q.m[0] / 2);
+        g->fast[1] = !generic && axis2_supported(q.m[1]) && (size_t)q.lanes == lanes_full;
+        g->fast[2] = !generic && zmul2_supported(q.m[2]) && (size_t)q.lanes == lanes_full;
+    }
     g->dirty = true;
     g->mixed = 0;
     g->map = nullptr;
@@ -462,18 +473,30 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     const T* Kt = reinterpret_cast<const T*>(g->ws + g->o_Kt);
     const int64_t p = q.pitch;
     const int slabs = B * 3 * q.n[2];
+    const int64_t rows = (int64_t)slabs * q.n[1];
     mark(g, K_XFWD, st);
-    FE_CUDA(launch_xfwd<T>(g->ctx, Y, S1, q.n[0], q.n[1], slabs, q.n[0], (int64_t)q.n[0] * q.n[1], p, p * q.n[1], st));
+    if (g->fast[0]) FE_CUDA(launch_xfwd2<T>(g->ctx, Y, S1, q.n[0], rows, q.n[0], p, st));
+    else FE_CUDA(launch_xfwd<T>(g->ctx, Y, S1, q.n[0], q.n[1], slabs, q.n[0], (int64_t)q.n[0] * q.n[1], p, p * q.n[1], st));
     mark(g, K_YFWD, st);
-    FE_CUDA(launch_axis<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.n[1],
-                           p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
+    if (g->fast[1])
+        FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.pitch, q.n[2], B * 3, p, p * q.n[1],
+                                p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
+    else
+        FE_CUDA(launch_axis<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.n[1],
+                               p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
     mark(g, K_ZMUL, st);
-    FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
+    if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.pitch, B, st));
+    else FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
     mark(g, K_YINV, st);
-    FE_CUDA(launch_axis<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.m[1],
-                           p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
+    if (g->fast[1])
+        FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.pitch, q.n[2], B * 3, p, p * q.m[1],
+                                p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
+    else
+        FE_CUDA(launch_axis<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.m[1],
+                               p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
     mark(g, K_XINV, st);
-    FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
+    if (g->fast[0]) FE_CUDA(launch_xinv2<T>(g->ctx, S1, E, q.n[0], rows, p, q.n[0], st));
+    else FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
     g->launches += 5;
     return FE_OK;
 }

@@ -1,0 +1,225 @@
+// fe_fft2_x.cu -- size-specialised x passes: real rows of n_x
+// values (zero-padded to m_x = 2 M when the axis is open) <-> half spectra X[0..M].
+// The real transform of length 2 M runs as a complex transform of length M on z[j] = x[2j] + i x[2j+1]:
+//   forward  Z = FFT_M(z);  X[k] = (Z[k] + conj Z[M-k])/2 - (i/2) w_2M^k (Z[k] - conj Z[M-k])
+//   inverse  Z[k] = (X[k] + conj X[M-k])/2 + (i/2) conj(w_2M^k) (X[k] - conj X[M-k]);  z = M * IFFT_M(Z)
+// (the inverse is unnormalised; 1/(M m_y m_z) is folded into the tensor spectrum at precompute).
+// Each row is handled by R2 threads with the register two-level transform of fe_fft2.cuh.
+#include "fe_fft2.cuh"
+
+namespace fe {
+namespace v2 {
+
+struct X2Args {
+    const void* tw;
+    int64_t nrows;
+    int64_t real_rs, spec_rs;     // row strides in reals / complex elements
+};
+
+template <int M> struct XCfg {
+    static constexpr int R1 = Fact<M>::R1, R2 = Fact<M>::R2;
+    static constexpr int TPP = R2;
+    static constexpr int ROWS = 256 / TPP;            // rows per block (256 threads)
+    static constexpr int XPITCH = R1 * (R2 + 1);      // padded exchange layout idx(k1, n2) = k1 (R2+1) + n2
+    static constexpr int RPITCH = XPITCH > M + 1 ? XPITCH : M + 1;
+};
+
+template <typename T, int M, bool PRUNE>
+__global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __restrict__ in, cx<T>* __restrict__ out, X2Args a)
+{
+    using C = XCfg<M>;
+    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT3 = R1 / TPP;
+    cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);   // w_M^e
+    cx<T>* tws = tw + M;                              // w_2M^k, k < M
+    cx<T>* buf = tws + M;
+    const int tp = threadIdx.x % TPP, rl = threadIdx.x / TPP;
+    const int64_t row = (int64_t)blockIdx.x * C::ROWS + rl;
+    const bool live = row < a.nrows;
+    cx<T>* rb = buf + rl * C::RPITCH;
+
+    cx<T> v[R1];
+    constexpr int NLOAD = PRUNE ? R1 / 2 : R1;
+    if (live) {
+        const cx<T>* src = reinterpret_cast<const cx<T>*>(in + row * a.real_rs) + tp;
+        static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = src[R2 * decltype(ic)::value]; });
+    } else {
+        static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = cx<T>{0, 0}; });
+    }
+    {
+        const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
+        for (int e = threadIdx.x; e < M; e += 256) {
+            tw[e] = twg[e * (kTwiddleN / M)];
+            tws[e] = twg[e * (kTwiddleN / (2 * M))];
+        }
+    }
+    __syncthreads();
+    Dif<T, -1, R1, 0, PRUNE>::run(v);
+    static_for<R1>([&](auto pc) {
+        constexpr int p = decltype(pc)::value;
+        constexpr int k1 = brev<R1>(p);
+        cx<T> val = v[p];
+        if constexpr (k1 != 0) val = cmul(val, tw[tp * k1]);
+        rb[k1 * (R2 + 1) + tp] = val;
+    });
+    __syncthreads();
+    cx<T> u[NT3][R2];
+#pragma unroll
+    for (int it = 0; it < NT3; ++it) {
+        const int k1 = tp + it * TPP;
+        static_for<R2>([&](auto nc) { u[it][decltype(nc)::value] = rb[k1 * (R2 + 1) + decltype(nc)::value]; });
+        Dif<T, -1, R2>::run(u[it]);
+    }
+    __syncthreads();     // exchange layout fully read; reuse the row buffer in natural order
+#pragma unroll
+    for (int it = 0; it < NT3; ++it) {
+        const int k1 = tp + it * TPP;
+        static_for<R2>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            rb[k1 + R1 * brev<R2>(p)] = u[it][p];
+        });
+    }
+    __syncthreads();
+    if (live) {
+        cx<T>* dst = out + row * a.spec_rs;
+        for (int k = tp; k <= M / 2; k += TPP) {
+            const cx<T> Zk = rb[k], Zn = rb[(M - k) & (M - 1)];
+            const T ex = (T)0.5 * (Zk.x + Zn.x), ey = (T)0.5 * (Zk.y - Zn.y);
+            const T ox = (T)0.5 * (Zk.y + Zn.y), oy = (T)-0.5 * (Zk.x - Zn.x);
+            const cx<T> w = tws[k];
+            // X[k] = Xe + w Xo;  X[M-k] = conj(Xe) - conj(w Xo)   (w_2M^(M-k) = -conj(w_2M^k), Xo(M-k) = conj Xo(k))
+            const T px = ox * w.x - oy * w.y, py = ox * w.y + oy * w.x;
+            dst[k] = {ex + px, ey + py};
+            dst[M - k] = {ex - px, py - ey};
+        }
+    }
+}
+
+template <typename T, int M, bool PRUNE>
+__global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __restrict__ in, T* __restrict__ out, X2Args a)
+{
+    using C = XCfg<M>;
+    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT3 = R1 / TPP;
+    cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);
+    cx<T>* tws = tw + M;
+    cx<T>* buf = tws + M;
+    const int tp = threadIdx.x % TPP, rl = threadIdx.x / TPP;
+    const int64_t row = (int64_t)blockIdx.x * C::ROWS + rl;
+    const bool live = row < a.nrows;
+    cx<T>* rb = buf + rl * C::RPITCH;
+
+    {
+        const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
+        for (int e = threadIdx.x; e < M; e += 256) {
+            tw[e] = twg[e * (kTwiddleN / M)];
+            tws[e] = twg[e * (kTwiddleN / (2 * M))];
+        }
+    }
+    __syncthreads();
+    cx<T> v[R1];
+    const cx<T>* src = in + (live ? row : 0) * a.spec_rs;
+    static_for<R1>([&](auto jc) {
+        constexpr int j1 = decltype(jc)::value;
+        const int k = tp + R2 * j1;
+        const cx<T> Xk = src[k], Xn = src[M - k];
+        const T ex = (T)0.5 * (Xk.x + Xn.x), ey = (T)0.5 * (Xk.y - Xn.y);
+        const T dx = (T)0.5 * (Xk.x - Xn.x), dy = (T)0.5 * (Xk.y + Xn.y);
+        const cx<T> w = tws[k];
+        const T ox = dx * w.x + dy * w.y, oy = dy * w.x - dx * w.y;   // D * conj(w)
+        v[j1] = {ex - oy, ey + ox};
+    });
+    Dif<T, +1, R1>::run(v);
+    static_for<R1>([&](auto pc) {
+        constexpr int p = decltype(pc)::value;
+        constexpr int o1 = brev<R1>(p);
+        cx<T> val = v[p];
+        if constexpr (o1 != 0) val = cmulc(val, tw[tp * o1]);
+        rb[o1 * (R2 + 1) + tp] = val;
+    });
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < NT3; ++it) {
+        const int o1 = tp + it * TPP;
+        cx<T> u[R2];
+        static_for<R2>([&](auto nc) { u[decltype(nc)::value] = rb[o1 * (R2 + 1) + decltype(nc)::value]; });
+        Dif<T, +1, R2>::run(u);
+        if (live) {
+            cx<T>* dst = reinterpret_cast<cx<T>*>(out + row * a.real_rs) + o1;
+            static_for<R2>([&](auto pc) {
+                constexpr int p = decltype(pc)::value;
+                constexpr int o2 = brev<R2>(p);
+                if constexpr (!PRUNE || o2 < R2 / 2) dst[R1 * o2] = u[p];
+            });
+        }
+    }
+}
+
+template <typename T, int M, bool PRUNE, bool FWD>
+static cudaError_t launch_one(const void* in, void* out, const X2Args& a, cudaStream_t st)
+{
+    using C = XCfg<M>;
+    constexpr size_t smem = (size_t)(2 * M + C::ROWS * C::RPITCH) * sizeof(cx<T>);
+    static bool configured = false;
+    const dim3 grid((unsigned)((a.nrows + C::ROWS - 1) / C::ROWS));
+    if constexpr (FWD) {
+        if (!configured) {
+            cudaError_t e = cudaFuncSetAttribute(k2_xfwd<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            configured = true;
+        }
+        k2_xfwd<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
+    } else {
+        if (!configured) {
+            cudaError_t e = cudaFuncSetAttribute(k2_xinv<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            configured = true;
+        }
+        k2_xinv<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<const cx<T>*>(in), static_cast<T*>(out), a);
+    }
+    return cudaGetLastError();
+}
+
+template <typename T, bool FWD>
+static cudaError_t launch_x(int M, bool prune, const void* in, void* out, const X2Args& a, cudaStream_t st)
+{
+    switch (M) {
+        case 64: return prune ? launch_one<T, 64, true, FWD>(in, out, a, st) : launch_one<T, 64, false, FWD>(in, out, a, st);
+        case 128: return prune ? launch_one<T, 128, true, FWD>(in, out, a, st) : launch_one<T, 128, false, FWD>(in, out, a, st);
+        case 256: return prune ? launch_one<T, 256, true, FWD>(in, out, a, st) : launch_one<T, 256, false, FWD>(in, out, a, st);
+        case 512: return prune ? launch_one<T, 512, true, FWD>(in, out, a, st) : launch_one<T, 512, false, FWD>(in, out, a, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace v2
+
+bool x2_supported(int Mc) { return Mc == 64 || Mc == 128 || Mc == 256 || Mc == 512; }
+
+// nrows uniformly strided rows: n_real valid reals per row (n_real == 2 Mc, or Mc when zero-padded)
+template <typename T>
+cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, int64_t nrows, int64_t real_rs,
+                         int64_t spec_rs, cudaStream_t st)
+{
+    const int M = c.plan[0].M;
+    const bool prune = n_real == M;
+    if (!prune && n_real != 2 * M) return cudaErrorInvalidValue;
+    v2::X2Args a{c.tw, nrows, real_rs, spec_rs};
+    return v2::launch_x<T, true>(M, prune, in, out, a, st);
+}
+
+template <typename T>
+cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t spec_rs,
+                         int64_t real_rs, cudaStream_t st)
+{
+    const int M = c.plan[0].M;
+    const bool prune = n_real == M;
+    if (!prune && n_real != 2 * M) return cudaErrorInvalidValue;
+    v2::X2Args a{c.tw, nrows, real_rs, spec_rs};
+    return v2::launch_x<T, false>(M, prune, in, out, a, st);
+}
+
+template cudaError_t launch_xfwd2<double>(const FftCtx&, const double*, void*, int, int64_t, int64_t, int64_t, cudaStream_t);
+template cudaError_t launch_xfwd2<float>(const FftCtx&, const float*, void*, int, int64_t, int64_t, int64_t, cudaStream_t);
+template cudaError_t launch_xinv2<double>(const FftCtx&, const void*, double*, int, int64_t, int64_t, int64_t, cudaStream_t);
+template cudaError_t launch_xinv2<float>(const FftCtx&, const void*, float*, int, int64_t, int64_t, int64_t, cudaStream_t);
+
+}  // namespace fe

@@ -89,6 +89,24 @@ template <typename T>
 cudaError_t launch_extract(const void* Sbox, T* Kt_comp, int Mz, int My, int Lx, int pitch64, int pitchT,
                            double scale, cudaStream_t st);
 size_t zmul_smem_bytes(int Mz, int lanes, size_t cx_bytes);
+
+// ---- size-specialised register FFT passes (fe_fft2_*.cu); same data layouts as the generic launchers above
+bool x2_supported(int Mc);
+bool axis2_supported(int M);
+bool zmul2_supported(int M);
+template <typename T>
+cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, int64_t nrows, int64_t real_rs,
+                         int64_t spec_rs, cudaStream_t st);
+template <typename T>
+cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t spec_rs,
+                         int64_t real_rs, cudaStream_t st);
+template <typename T>
+cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int pitch_used,
+                         int outer, int batch, int64_t in_sa, int64_t in_so, int64_t in_sb, int64_t out_sa,
+                         int64_t out_so, int64_t out_sb, cudaStream_t st);
+template <typename T>
+cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int pitch,
+                         int batch, cudaStream_t st);
 cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
 
 // ---- tensor (fe_tensor.cu) --------------------------------------------------------------------

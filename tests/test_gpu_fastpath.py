@@ -1,0 +1,148 @@
+"""-m gpu parity tests of the size-specialised register FFT passes (fe_fft2_*.cu): grids large enough that every
+axis takes the fast kernels (transform lengths 64 / 128 / 256 / 512, pruned and unpruned), against the CPU oracle
+(oracle-FFT O8, itself pinned to the direct sum), and full-size checks of configs 5a / 5b against the closed-form
+tensor entry, one sampled output at a time."""
+import numpy as np
+import pytest
+
+import fe_inputs as fi
+from oracle import fe_oracle as orc
+from gpu_util import rel_l2, oracle_problem
+
+pytestmark = pytest.mark.gpu
+
+TOL_RHS64, TOL32 = 1e-10, 1e-4
+
+
+@pytest.fixture(scope="module")
+def fe():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2605_28800_b200 as fe
+    fe.load()
+    return fe
+
+
+def _workload(n, periodic=(0, 0, 0), images=(0, 0, 0), batch=1, seed=77):
+    w = fi.open_batio3("fast_%dx%dx%d" % n, n, batch, "f64", seed)
+    w.periodic, w.pbc_images = tuple(periodic), tuple(images)
+    return w
+
+
+# padded lengths (Mc = m_x / 2, m_y, m_z) exercised:            x     y     z
+@pytest.mark.parametrize("n,periodic,images", [
+    ((64, 32, 32), (0, 0, 0), (0, 0, 0)),        #  64p   64p   64p
+    ((128, 64, 32), (0, 0, 0), (0, 0, 0)),       # 128p  128p   64p
+    ((256, 128, 64), (0, 0, 0), (0, 0, 0)),      # 256p  256p  128p
+    ((32, 256, 128), (0, 0, 0), (0, 0, 0)),      # generic 512p 256p
+    ((512, 32, 32), (0, 0, 0), (0, 0, 0)),       # 512p   64p   64p
+    ((128, 64, 32), (1, 1, 0), (1, 1, 0)),       #  64    64    64p  (unpruned x, y)
+    ((64, 64, 64), (0, 0, 1), (0, 0, 1)),        #  64p  128p   64   (unpruned z)
+    ((256, 128, 16), (1, 1, 0), (1, 1, 0)),      # 128   128   generic
+])
+def test_fast_passes_against_oracle_fft(fe, n, periodic, images):
+    w = _workload(n, periodic, images)
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    o = orc.Oracle(oracle_problem(w), elec="fft")
+    P = g.state(w.P0)
+    got = g.rhs(P, fi.TERM_ELEC).cpu().numpy()[0]
+    want = o.rhs(w.P0[0], fi.TERM_ELEC)
+    assert rel_l2(got, want) < TOL_RHS64
+    got = g.rhs(P, fi.TERM_ALL).cpu().numpy()[0]
+    want = o.rhs(w.P0[0], fi.TERM_ALL)
+    assert rel_l2(got, want) < TOL_RHS64
+    # sampled outputs against the O(N) direct sum per target (not the FFT)
+    rng = np.random.default_rng(3)
+    t = rng.integers(0, w.cells, size=6)
+    Ed = orc.field_direct(o.p, o.table(), w.P0[0], targets=t)
+    got_e = g.rhs(P, fi.TERM_ELEC).cpu().numpy()[0].reshape(3, -1)[:, t] / w.globals_[0].L
+    assert np.max(np.abs(got_e - Ed)) < 1e-10 * np.max(np.abs(Ed))
+    g.close()
+
+
+def test_fast_passes_batch_and_fp32(fe):
+    w = _workload((128, 64, 32), batch=3)
+    o = [orc.Oracle(oracle_problem(w, b), elec="fft") for b in range(3)]
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    got = g.rhs(g.state(w.P0)).cpu().numpy()
+    for b in range(3):
+        assert rel_l2(got[b], o[b].rhs(w.P0[b])) < TOL_RHS64
+    g.close()
+    g = fe.Grid.from_workload(w, dtype="f32")
+    g.precompute_tensor()
+    P32 = w.P0.astype(np.float32)
+    got = g.rhs(g.state(P32)).cpu().numpy()
+    for b in range(3):
+        assert rel_l2(got[b], o[b].rhs(P32[b].astype(np.float64))) < TOL32
+    g.close()
+
+
+def test_fast_passes_steps_and_energy(fe):
+    """10 Euler steps and 3 RK4 steps on a grid that takes the fast kernels; energies against the oracle."""
+    w = _workload((64, 32, 32))
+    o = orc.Oracle(oracle_problem(w), elec="fft")
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    g.step(P, w.dt, 10, fi.EULER, fi.TERM_ALL)
+    ref = o.step(w.P0[0], w.dt, 10, fi.EULER, fi.TERM_ALL)
+    assert rel_l2(P.cpu().numpy()[0], ref) < 1e-11
+    e, eo = g.energy(P)[0], o.energy(ref)
+    assert np.allclose(e[:5], eo[:5], rtol=1e-9, atol=1e-10 * abs(eo[4]))
+    g.step(P, 2 * w.dt, 3, fi.RK4, fi.TERM_ALL)
+    ref = o.step(ref, 2 * w.dt, 3, fi.RK4, fi.TERM_ALL)
+    assert rel_l2(P.cpu().numpy()[0], ref) < 1e-11
+    g.close()
+
+
+@pytest.mark.parametrize("cfg,dtype,tol", [("5a", "f64", 1e-10), ("5a", "f32", 1e-4), ("5b", "f64", 1e-10)])
+def test_full_size_point_sources_against_closed_form(fe, cfg, dtype, tol):
+    """Full-size configs 5a / 5b in the launch configuration bench.py times.  P = a few single polarised cells
+    (corners, centre, random) => E_i(r) = -scale sum_s K_ij(r - r_s) p_s,j, with K from the oracle's closed form
+    (orc.newell_entry), evaluated at sampled output cells one by one."""
+    import torch
+    w = fi.config5a(dtype) if cfg == "5a" else fi.config5b(dtype)
+    nx, ny, nz = w.n
+    g = fe.Grid.from_workload(w, dtype=dtype)
+    g.precompute_tensor()
+    rng = np.random.default_rng(11)
+    src = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (nx // 2, ny // 2, nz // 2), (nx - 1, 0, nz // 3)]
+    src += [tuple(int(rng.integers(0, m)) for m in w.n) for _ in range(3)]
+    amp = rng.standard_normal((len(src), 3))
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    P = torch.zeros((w.batch, 3, nz, ny, nx), dtype=tdt, device="cuda:0")
+    b = w.batch - 1
+    for s, a in zip(src, amp):
+        for c in range(3):
+            P[b, c, s[2], s[1], s[0]] = float(a[c])
+    if dtype == "f32":
+        amp = amp.astype(np.float32).astype(np.float64)
+    E = g.rhs(P, fi.TERM_ELEC)[b].cpu().numpy().astype(np.float64) / w.globals_[b].L
+    gl = w.globals_[b]
+    scale = 1.0 / (gl.eps0 * gl.epsB)
+    cidx = ((0, 3, 4), (3, 1, 5), (4, 5, 2))
+    targets = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (1, 0, 0), (nx // 2, ny // 2 + 1, nz // 2)]
+    targets += [tuple(int(rng.integers(0, m)) for m in w.n) for _ in range(8)]
+    targets += [(min(s[0] + 1, nx - 1), s[1], s[2]) for s in src]
+    emax = 0.0
+    errs = []
+    for t in targets:
+        want = np.zeros(3)
+        for s, a in zip(src, amp):
+            off = (t[0] - s[0], t[1] - s[1], t[2] - s[2])
+            K = [orc.newell_entry(c6, off, w.d) for c6 in range(6)]
+            for i in range(3):
+                want[i] -= scale * sum(K[cidx[i][j]] * a[j] for j in range(3))
+        got = E[:, t[2], t[1], t[0]]
+        errs.append(np.max(np.abs(got - want)))
+        emax = max(emax, np.max(np.abs(want)))
+    # far-field entries are ~1e-8 of the self term: the bound is relative to the largest sampled field
+    assert max(errs) < tol * emax, (max(errs), emax)
+    # linearity / finiteness everywhere
+    assert np.isfinite(E).all()
+    if w.batch > 1:
+        assert float(g.rhs(P, fi.TERM_ELEC)[0].abs().max()) == 0.0      # other members untouched
+    g.close()
