@@ -135,6 +135,10 @@ struct LocalArgs {
     uint32_t terms;
     int batch;
     int mixed;            // any member has Gm != 0
+    // filled by launch_local
+    double id2[3];        // 1 / D_a^2
+    double i4[3];         // 1 / (4 D_x D_y), 1 / (4 D_x D_z), 1 / (4 D_y D_z)
+    int zchunk;           // planes per block
 };
 template <typename T> cudaError_t launch_local(const LocalArgs& a, cudaStream_t st);
 

@@ -71,119 +71,224 @@ struct Grid {
     }
 };
 
+// ------------------------------------------------------------------------------------------------
+// k_local: one block owns a 32 x 8 column of cells and marches along z.  The three components of the
+// current plane and its two z neighbours live in a 4-slot ring of shared-memory tiles with a one-cell halo
+// (zero outside the sample / in vacuum cells, wrapped on periodic axes) plus one validity byte per cell, so
+// every P value is fetched from global memory once per block and all 7 / 19 stencil taps come from shared
+// memory.  One __syncthreads per plane: the plane z+1 is loaded into the slot that held z-3.
+// ------------------------------------------------------------------------------------------------
+constexpr int kTX = 32, kTY = 8, kHX = kTX + 2, kHY = kTY + 2, kTile = kHX * kHY;   // 34 x 10 = 340
+constexpr int kNL = (3 * kTile + 255) / 256;                                        // loader entries per thread
+
 template <typename T, bool MAP, bool MIXED>
 __global__ void __launch_bounds__(256) k_local(LocalArgs a)
 {
+    extern __shared__ __align__(16) unsigned char lsm[];
+    T* tiles = reinterpret_cast<T*>(lsm);                                   // [4][3][kTile]
+    unsigned char* flags = lsm + (size_t)4 * 3 * kTile * sizeof(T);         // [4][kTile]
+    LandauT<T>* smats = reinterpret_cast<LandauT<T>*>(flags + 4 * kTile + 8);  // [nmat]  (offset is 16-aligned)
+    unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
+
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int yz = blockIdx.y;
-    const int y = yz % ny, z = yz / ny;
+    const int ntx = (nx + kTX - 1) / kTX;
+    const int x0 = (blockIdx.x % ntx) * kTX, y0 = (blockIdx.x / ntx) * kTY;
+    const int z0 = blockIdx.y * a.zchunk, z1 = min(z0 + a.zchunk, nz);
     const int b = blockIdx.z;
-    if (x >= nx) return;
-    const int64_t N = (int64_t)nx * ny * nz;
-    const int64_t r = ((int64_t)z * ny + y) * nx + x;
+    const int t = threadIdx.x, tx = t & 31, ty = t >> 5;
+    const int64_t nxy = (int64_t)nx * ny, N = nxy * nz;
     const T* Y = static_cast<const T*>(a.Y) + (int64_t)b * 3 * N;
     const DevLandau* mats = a.mats + (int64_t)b * a.nmat;
-    const DevMember mem = a.members[b];
-    const int mat = MAP ? a.map[r] : 0;
-    const bool act = mats[mat].active != 0;
-
-    T k[3] = {0, 0, 0};
-    if (act) {
-        const T p0[3] = {Y[r], Y[N + r], Y[2 * N + r]};
-        T E[3] = {0, 0, 0};
-        if (a.terms & 1u) {
-            const LandauT<T> L(mats[mat]);
-            const T A = p0[0] * p0[0], B = p0[1] * p0[1], C = p0[2] * p0[2];
-            E[0] -= p0[0] * L.dfd(L.a1x, A, B, C);
-            E[1] -= p0[1] * L.dfd(L.a1y, B, C, A);
-            E[2] -= p0[2] * L.dfd(L.a1z, C, A, B);
-        }
-        if (a.terms & 2u) {
-            Grid<T, MAP> g{{Y, Y + N, Y + 2 * N}, a.map, mats, nx, ny, nz};
-            const int c0[3] = {x, y, z};
-            const T G11 = (T)mem.G11, Gt = (T)mem.Gt;
-            const T id2[3] = {(T)(1.0 / (a.d[0] * a.d[0])), (T)(1.0 / (a.d[1] * a.d[1])), (T)(1.0 / (a.d[2] * a.d[2]))};
-#pragma unroll
-            for (int ax = 0; ax < 3; ++ax) {
-#pragma unroll
-                for (int s = -1; s <= 1; s += 2) {
-                    int q[3] = {c0[0], c0[1], c0[2]};
-                    q[ax] = nb(c0[ax], s, a.n[ax], a.periodic[ax]);
-                    bool ok;
-                    const T vx = g.val(0, q[0], q[1], q[2], ok);
-                    if (ok) {
-                        const T vy = g.p[1][((int64_t)q[2] * ny + q[1]) * nx + q[0]];
-                        const T vz = g.p[2][((int64_t)q[2] * ny + q[1]) * nx + q[0]];
-                        E[0] += (ax == 0 ? G11 : Gt) * id2[ax] * (vx - p0[0]);
-                        E[1] += (ax == 1 ? G11 : Gt) * id2[ax] * (vy - p0[1]);
-                        E[2] += (ax == 2 ? G11 : Gt) * id2[ax] * (vz - p0[2]);
-                    }
-                }
-            }
-            if (MIXED) {
-                const T Gm = (T)mem.Gm;
-                if (Gm != (T)0) {
-#pragma unroll
-                    for (int i = 0; i < 3; ++i) {
-                        T acc = 0;
-#pragma unroll
-                        for (int j = 0; j < 3; ++j) {
-                            if (j == i) continue;
-                            T t = 0;
-#pragma unroll
-                            for (int si = -1; si <= 1; si += 2) {
-                                const int ci = nb(c0[i], si, a.n[i], a.periodic[i]);
-                                if (ci < 0) continue;      // intermediate cell must be inside the grid
-                                int qp[3] = {c0[0], c0[1], c0[2]}, qm[3] = {c0[0], c0[1], c0[2]};
-                                qp[i] = ci; qm[i] = ci;
-                                qp[j] = nb(c0[j], +1, a.n[j], a.periodic[j]);
-                                qm[j] = nb(c0[j], -1, a.n[j], a.periodic[j]);
-                                const T up = g.val(j, qp[0], qp[1], qp[2]);
-                                const T dn = g.val(j, qm[0], qm[1], qm[2]);
-                                t += (T)si * (up - dn);
-                            }
-                            acc += t * (T)(0.25 / (a.d[i] * a.d[j]));
-                        }
-                        E[i] += Gm * acc;
-                    }
-                }
-            }
-        }
-        if ((a.terms & 4u) && a.Eelec) {
-            const T* Ee = static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N;
-            E[0] += Ee[r]; E[1] += Ee[N + r]; E[2] += Ee[2 * N + r];
-        }
-        if (a.terms & 8u) {
-            E[0] += (T)mem.Eext[0]; E[1] += (T)mem.Eext[1]; E[2] += (T)mem.Eext[2];
-        }
-        const T L = (T)mem.L;
-        k[0] = L * E[0]; k[1] = L * E[1]; k[2] = L * E[2];
+    for (int m = t; m < a.nmat; m += 256) {
+        smats[m] = LandauT<T>(mats[m]);
+        sact[m] = mats[m].active != 0;
     }
-    T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
+    const DevMember mem = a.members[b];
+
+    // loader entries: shared offset, in-plane global offset (-1: outside an open axis), component
+    int l_so[kNL], l_go[kNL];
+#pragma unroll
+    for (int k = 0; k < kNL; ++k) {
+        const int idx = t + 256 * k;
+        l_so[k] = -1;
+        l_go[k] = -1;
+        if (idx < 3 * kTile) {
+            const int rem = idx % kTile, yy = rem / kHX, xx = rem % kHX;
+            int gx = x0 - 1 + xx, gy = y0 - 1 + yy;
+            bool in = true;
+            if (gx < 0 || gx >= nx) { if (a.periodic[0]) gx = ((gx % nx) + nx) % nx; else in = false; }
+            if (gy < 0 || gy >= ny) { if (a.periodic[1]) gy = ((gy % ny) + ny) % ny; else in = false; }
+            l_so[k] = idx;
+            l_go[k] = in ? gy * nx + gx : -1;
+        }
+    }
+    // global -> registers (issued one plane ahead of its use), registers -> shared tile
+    T pre[kNL];
+    bool pok[kNL];
+    auto fetch_plane = [&](int z) {
+        int zz = z;
+        bool zin = true;
+        if (zz < 0 || zz >= nz) { if (a.periodic[2]) zz = ((zz % nz) + nz) % nz; else zin = false; }
+#pragma unroll
+        for (int k = 0; k < kNL; ++k) {
+            const bool ok = zin && l_go[k] >= 0;
+            const int64_t r = (int64_t)zz * nxy + l_go[k];
+            pre[k] = ok ? Y[(l_so[k] / kTile) * N + r] : (T)0;
+            pok[k] = ok;
+            if (MAP) { if (ok) pok[k] = sact[a.map[r]] != 0; }
+        }
+    };
+    auto store_plane = [&](int z) {
+        const int slot = z & 3;
+        T* tl = tiles + slot * 3 * kTile;
+        unsigned char* fl = flags + slot * kTile;
+#pragma unroll
+        for (int k = 0; k < kNL; ++k) {
+            if (l_so[k] < 0) continue;
+            tl[l_so[k]] = pok[k] ? pre[k] : (T)0;
+            if (l_so[k] < kTile) fl[l_so[k]] = pok[k];
+        }
+    };
+    __syncthreads();          // coefficient tables visible (fetch_plane reads sact)
+    fetch_plane(z0 - 1);
+    store_plane(z0 - 1);
+    fetch_plane(z0);
+    store_plane(z0);
+    fetch_plane(z0 + 1);
+
+    const int x = x0 + tx, y = y0 + ty;
+    const bool inside = x < nx && y < ny;
+    const int64_t rxy = (int64_t)y * nx + x;
+    const int c0 = (ty + 1) * kHX + tx + 1;
+    const T G11 = (T)mem.G11, Gt = (T)mem.Gt, Gm = (T)mem.Gm, L = (T)mem.L;
+    const T ix = (T)a.id2[0], iy = (T)a.id2[1], iz = (T)a.id2[2];
+    const T qxy = Gm * (T)a.i4[0], qxz = Gm * (T)a.i4[1], qyz = Gm * (T)a.i4[2];
+    const T cy = (T)a.cy, ca = (T)a.ca;
+    const T ex0 = (T)mem.Eext[0], ex1 = (T)mem.Eext[1], ex2 = (T)mem.Eext[2];
+    const T* Ee = (a.terms & 4u) && a.Eelec ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
     const T* base = a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
-    const T cy = (T)a.cy;
+    const bool base_is_Y = a.baseY == a.Y;
+    T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
+    const T* ai = a.accOut ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
+    T* ao = a.accOut ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
+    LandauT<T> lc0 = smats[0];
+
+    T en[3] = {0, 0, 0};
+    if (Ee && inside) {
+        const int64_t r = (int64_t)z0 * nxy + rxy;
+        en[0] = Ee[r]; en[1] = Ee[N + r]; en[2] = Ee[2 * N + r];
+    }
+    for (int z = z0; z < z1; ++z) {
+        store_plane(z + 1);
+        __syncthreads();
+        if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
+        if (!inside) continue;
+        const T ec[3] = {en[0], en[1], en[2]};
+        if (Ee && z + 1 < z1) {
+            const int64_t rn = (int64_t)(z + 1) * nxy + rxy;
+            en[0] = Ee[rn]; en[1] = Ee[N + rn]; en[2] = Ee[2 * N + rn];
+        }
+        const T* m0 = tiles + ((z - 1) & 3) * 3 * kTile;      // plane z-1
+        const T* c = tiles + (z & 3) * 3 * kTile;             // plane z
+        const T* p1 = tiles + ((z + 1) & 3) * 3 * kTile;      // plane z+1
+        const unsigned char* fm = flags + ((z - 1) & 3) * kTile;
+        const unsigned char* fc = flags + (z & 3) * kTile;
+        const unsigned char* fp = flags + ((z + 1) & 3) * kTile;
+        const int64_t r = (int64_t)z * nxy + rxy;
+        T k[3] = {0, 0, 0};
+        if (fc[c0]) {
+            const T px = c[c0], py = c[kTile + c0], pz = c[2 * kTile + c0];
+            T E0 = 0, E1 = 0, E2 = 0;
+            if (a.terms & 1u) {
+                const LandauT<T> lc = MAP ? smats[a.map[r]] : lc0;
+                const T A = px * px, B = py * py, C = pz * pz;
+                E0 -= px * lc.dfd(lc.a1x, A, B, C);
+                E1 -= py * lc.dfd(lc.a1y, B, C, A);
+                E2 -= pz * lc.dfd(lc.a1z, C, A, B);
+            }
+            if (a.terms & 2u) {
+                // bonds: sum over existing neighbours of c_ia / D_a^2 (P_i(nb) - P_i(r)); a missing neighbour holds 0
+                const T nxf = (T)(fc[c0 - 1] + fc[c0 + 1]), nyf = (T)(fc[c0 - kHX] + fc[c0 + kHX]);
+                const T nzf = (T)(fm[c0] + fp[c0]);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) Yout[c * N + r] = (base ? base[c * N + r] : (T)0) + cy * k[c];
-    if (a.accOut) {
-        const T* ai = static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N;
-        T* ao = static_cast<T*>(a.accOut) + (int64_t)b * 3 * N;
-        const T ca = (T)a.ca;
+                for (int i = 0; i < 3; ++i) {
+                    const T* ci = c + i * kTile;
+                    const T p = ci[c0];
+                    const T sx = ci[c0 - 1] + ci[c0 + 1] - nxf * p;
+                    const T sy = ci[c0 - kHX] + ci[c0 + kHX] - nyf * p;
+                    const T sz = m0[i * kTile + c0] + p1[i * kTile + c0] - nzf * p;
+                    const T e = (i == 0 ? G11 : Gt) * ix * sx + (i == 1 ? G11 : Gt) * iy * sy + (i == 2 ? G11 : Gt) * iz * sz;
+                    if (i == 0) E0 += e; else if (i == 1) E1 += e; else E2 += e;
+                }
+                if (MIXED) {
+                    // Gm sum_{j != i} [P_j(+i+j) - P_j(+i-j) - P_j(-i+j) + P_j(-i-j)] / (4 D_i D_j)
+                    const T* cx_ = c;               // Px plane z
+                    const T* cy_ = c + kTile;       // Py
+                    const T* cz_ = c + 2 * kTile;   // Pz
+                    const T dxy_y = cy_[c0 + 1 + kHX] - cy_[c0 + 1 - kHX] - cy_[c0 - 1 + kHX] + cy_[c0 - 1 - kHX];
+                    const T dxy_x = cx_[c0 + 1 + kHX] - cx_[c0 + 1 - kHX] - cx_[c0 - 1 + kHX] + cx_[c0 - 1 - kHX];
+                    const T dxz_z = p1[2 * kTile + c0 + 1] - m0[2 * kTile + c0 + 1] - p1[2 * kTile + c0 - 1] + m0[2 * kTile + c0 - 1];
+                    const T dxz_x = p1[c0 + 1] - m0[c0 + 1] - p1[c0 - 1] + m0[c0 - 1];
+                    const T dyz_z = p1[2 * kTile + c0 + kHX] - m0[2 * kTile + c0 + kHX] - p1[2 * kTile + c0 - kHX] + m0[2 * kTile + c0 - kHX];
+                    const T dyz_y = p1[kTile + c0 + kHX] - m0[kTile + c0 + kHX] - p1[kTile + c0 - kHX] + m0[kTile + c0 - kHX];
+                    E0 += qxy * dxy_y + qxz * dxz_z;
+                    E1 += qxy * dxy_x + qyz * dyz_z;
+                    E2 += qxz * dxz_x + qyz * dyz_y;
+                }
+            }
+            if (Ee) { E0 += ec[0]; E1 += ec[1]; E2 += ec[2]; }
+            if (a.terms & 8u) { E0 += ex0; E1 += ex1; E2 += ex2; }
+            k[0] = L * E0; k[1] = L * E1; k[2] = L * E2;
+        }
+        T bv[3] = {0, 0, 0};
+        if (base) {
+            if (base_is_Y) {
+                // the stage base is the state itself (Euler): take it from the tile; vacuum cells hold their raw value
+                if (fc[c0]) { bv[0] = c[c0]; bv[1] = c[kTile + c0]; bv[2] = c[2 * kTile + c0]; }
+                else { bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r]; }
+            } else {
+                bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r];
+            }
+        }
 #pragma unroll
-        for (int c = 0; c < 3; ++c) ao[c * N + r] = ai[c * N + r] + ca * k[c];
+        for (int i = 0; i < 3; ++i) Yout[i * N + r] = bv[i] + cy * k[i];
+        if (ao) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) ao[i * N + r] = ai[i * N + r] + ca * k[i];
+        }
     }
 }
 
-template <typename T> cudaError_t launch_local(const LocalArgs& a, cudaStream_t st)
+template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t st)
 {
-    const int bx = a.n[0] >= 256 ? 256 : (a.n[0] >= 128 ? 128 : (a.n[0] >= 64 ? 64 : 32));
-    dim3 grid((a.n[0] + bx - 1) / bx, a.n[1] * a.n[2], a.batch);
+    LocalArgs a = a0;
+    for (int i = 0; i < 3; ++i) a.id2[i] = 1.0 / (a.d[i] * a.d[i]);
+    a.i4[0] = 0.25 / (a.d[0] * a.d[1]);
+    a.i4[1] = 0.25 / (a.d[0] * a.d[2]);
+    a.i4[2] = 0.25 / (a.d[1] * a.d[2]);
+    const int ntx = (a.n[0] + kTX - 1) / kTX, nty = (a.n[1] + kTY - 1) / kTY;
+    // z chunk: as long as possible (halo planes are re-read per chunk) while the grid still fills the machine
+    int zc = a.n[2];
+    while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
+    a.zchunk = zc;
+    dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
+    const size_t smem = (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauT<T>) + 1);
+    static bool configured = false;
+    if (!configured) {
+        const int lim = 96 * 1024;      // 255 materials need 61 KB
+        cudaError_t e = cudaFuncSetAttribute(k_local<T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local<T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
     if (a.map) {
-        if (a.mixed) k_local<T, true, true><<<grid, bx, 0, st>>>(a);
-        else k_local<T, true, false><<<grid, bx, 0, st>>>(a);
+        if (a.mixed) k_local<T, true, true><<<grid, 256, smem, st>>>(a);
+        else k_local<T, true, false><<<grid, 256, smem, st>>>(a);
     } else {
-        if (a.mixed) k_local<T, false, true><<<grid, bx, 0, st>>>(a);
-        else k_local<T, false, false><<<grid, bx, 0, st>>>(a);
+        if (a.mixed) k_local<T, false, true><<<grid, 256, smem, st>>>(a);
+        else k_local<T, false, false><<<grid, 256, smem, st>>>(a);
     }
     return cudaGetLastError();
 }
