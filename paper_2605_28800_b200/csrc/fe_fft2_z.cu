@@ -3,180 +3,281 @@
 // on S[b][3][nz][My][pitch].  K~ is real and symmetric, stored for kz <= Mz/2, ky <= My/2; the odd components
 // change sign under ky -> -ky (xy, yz) and kz -> -kz (xz, yz).
 //
-// One thread holds the spectrum of all three components at the R2 frequencies kz = k1 + R1 k2 in registers, so
-// the multiply and the first stage of the inverse transform need no shared memory:
+// Persistent blocks, software pipelined with cp.async:
+//   work item  = (group of LANES consecutive kx, |ky|): the K~ tile of the item is copied to shared memory once and
+//                serves the tiles ky, My - ky of every batch member;
+//   tile       = LANES pencils x 3 components; its nz input rows are prefetched into a staging buffer while the
+//                previous tile is being transformed.
+// Per tile, one thread holds the spectrum of all three components at the R2 frequencies kz = k1 + R1 k2 in
+// registers, so the multiply and the first stage of the inverse transform need no shared-memory round trip:
 //   forward   x[n2 + R2 n1] -> (R1-point over n1) -> twiddle -> exchange -> (R2-point over n2) -> X[k1 + R1 k2]
 //   inverse   X[k1 + R1 k2] -> (R2-point over k2) -> twiddle -> exchange -> (R1-point over k1) -> x[n1 R2 + n2]
-// The thread that loaded rows n2 + R2 n1 stores exactly those rows again.
 #include "fe_fft2.cuh"
 
 namespace fe {
 namespace v2 {
 
+// factorisation used by the fused pass: R2 frequencies per thread (3 components in registers)
+template <int M> struct ZFact;
+template <> struct ZFact<64> { static constexpr int R1 = 8, R2 = 8; };
+template <> struct ZFact<128> { static constexpr int R1 = 16, R2 = 8; };
+template <> struct ZFact<256> { static constexpr int R1 = 32, R2 = 8; };
+
 struct Z2Args {
     const void* tw;
     const DevMember* members;
-    int My, pitch;
-    int nz;
+    int My, pitch, nz, batch;
+    int ngroups;      // pitch / LANES
+    int nitems;       // ngroups * (My/2 + 1)
 };
 
-template <typename T, int M, bool PRUNE>
-__global__ void __launch_bounds__((128 / (int)sizeof(cx<T>)) * Fact<M>::R1, 2)
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+template <typename T, int M, int LANES, bool PRUNE> struct ZCfg {
+    static constexpr int R1 = ZFact<M>::R1, R2 = ZFact<M>::R2;
+    static constexpr int TPP = R1;                          // threads per pencil (one step-3 task each)
+    static constexpr int THREADS = LANES * TPP;
+    static constexpr int NT1 = (3 * R2 + TPP - 1) / TPP;    // step-1 tasks (component, n2) per thread
+    static constexpr int TILE = M * LANES;                  // exchange tile of one component (complex)
+    static constexpr int NIN = PRUNE ? M / 2 : M;           // input rows per component
+    static constexpr int HZ = M / 2 + 1;
+    static constexpr size_t tw_bytes = (size_t)M * sizeof(cx<T>);
+    static constexpr size_t ex_bytes = (size_t)3 * TILE * sizeof(cx<T>);
+    static constexpr size_t st_bytes = (size_t)3 * NIN * LANES * sizeof(cx<T>);
+    static constexpr size_t k_bytes = ((size_t)6 * HZ * LANES * sizeof(T) + 15) / 16 * 16;
+    static constexpr size_t smem = tw_bytes + ex_bytes + st_bytes + k_bytes;
+};
+
+// position of a block in its sequence of tiles
+struct ZIter {
+    int item, t, nt;          // work item, tile within the item, tiles in the item
+    int kxg, kyh;
+    __device__ __forceinline__ void set_item(int it, const Z2Args& a)
+    {
+        item = it;
+        t = 0;
+        kxg = it % a.ngroups;
+        kyh = it / a.ngroups;
+        nt = a.batch * ((kyh == 0 || 2 * kyh == a.My) ? 1 : 2);
+    }
+    __device__ __forceinline__ bool valid(const Z2Args& a) const { return item < a.nitems; }
+    __device__ __forceinline__ void next(const Z2Args& a)
+    {
+        if (++t >= nt) set_item(item + gridDim.x, a);
+    }
+    // batch member and signed ky of the current tile
+    __device__ __forceinline__ void tile(const Z2Args& a, int& b, int& ky) const
+    {
+        const int nm = nt / a.batch;
+        b = t / nm;
+        ky = (t % nm) ? a.My - kyh : kyh;
+    }
+};
+
+template <typename T, int M, int LANES, bool PRUNE>
+__global__ void __launch_bounds__(ZCfg<T, M, LANES, PRUNE>::THREADS, 2)
 k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
 {
-    constexpr int R1 = Fact<M>::R1, R2 = Fact<M>::R2;
-    constexpr int LANES = 128 / (int)sizeof(cx<T>);
-    constexpr int TPP = R1;                                 // threads per pencil (one step-3 task each)
-    constexpr int NT1 = (3 * R2 + TPP - 1) / TPP;           // step-1 tasks (component, n2) per thread
-    constexpr int TILE = M * LANES;
+    using C = ZCfg<T, M, LANES, PRUNE>;
+    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT1 = C::NT1, TILE = C::TILE, NIN = C::NIN, HZ = C::HZ;
     constexpr int NLOAD = PRUNE ? R1 / 2 : R1;
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);
-    cx<T>* buf = tw + M;
+    cx<T>* buf = tw + M;                                            // exchange [3][M][LANES]
+    cx<T>* stage = buf + 3 * TILE;                                  // staged input [3][NIN][LANES]
+    T* kbuf = reinterpret_cast<T*>(stage + 3 * NIN * LANES);        // K~ tile [6][HZ][LANES]
     const int lane = threadIdx.x % LANES, tp = threadIdx.x / LANES;
-    const int kx0 = blockIdx.x * LANES, b = blockIdx.z;
-    // mirror pairs (ky, My - ky) are adjacent in launch order so that the second read of a K~ plane hits L2
-    const int yy = blockIdx.y;
-    const int ky = yy == 0 ? 0 : ((yy & 1) ? (yy + 1) >> 1 : a.My - (yy >> 1));
     const int64_t sa = (int64_t)a.My * a.pitch, cs = (int64_t)a.nz * sa;
-    cx<T>* base = S + (int64_t)b * 3 * cs + (int64_t)ky * a.pitch + kx0 + lane;
+    const int Hy = a.My / 2 + 1;
+    const int64_t kcs = (int64_t)HZ * Hy * a.pitch;
 
-    // ---- forward step 1: tasks (c, n2)
-    cx<T> v[NT1][NLOAD];
-#pragma unroll
-    for (int it = 0; it < NT1; ++it) {
-        const int task = tp + it * TPP;
-        if ((3 * R2) % TPP == 0 || task < 3 * R2) {
-            const int c = task / R2, n2 = task % R2;
-            const cx<T>* src = base + c * cs + (int64_t)n2 * sa;
-            static_for<NLOAD>([&](auto ic) {
-                constexpr int n1 = decltype(ic)::value;
-                v[it][n1] = src[(int64_t)(R2 * n1) * sa];
-            });
+    auto tile_base = [&](const ZIter& it) -> cx<T>* {
+        int b, ky;
+        it.tile(a, b, ky);
+        return S + (int64_t)b * 3 * cs + (int64_t)ky * a.pitch + it.kxg * LANES;
+    };
+    // asynchronous copies: input rows of a tile, K~ tile of an item
+    auto prefetch_tile = [&](const ZIter& it) {
+        const cx<T>* base = tile_base(it);
+        constexpr int PER16 = 16 / (int)sizeof(cx<T>);              // complex elements per 16-byte copy
+        constexpr int OPS_ROW = LANES / PER16, OPS = 3 * NIN * OPS_ROW;
+        for (int o = threadIdx.x; o < OPS; o += C::THREADS) {
+            const int q = o % OPS_ROW, row = (o / OPS_ROW) % NIN, c = o / (OPS_ROW * NIN);
+            cp_async16(stage + (c * NIN + row) * LANES + q * PER16, base + c * cs + (int64_t)row * sa + q * PER16);
         }
-    }
-    load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, LANES * TPP);
-    __syncthreads();
+    };
+    auto prefetch_k = [&](const ZIter& it) {
+        constexpr int PER16 = 16 / (int)sizeof(T);
+        constexpr int OPS_ROW = LANES / PER16, OPS = 6 * HZ * OPS_ROW;
+        const T* kb = Kt + (int64_t)it.kyh * a.pitch + it.kxg * LANES;
+        for (int o = threadIdx.x; o < OPS; o += C::THREADS) {
+            const int q = o % OPS_ROW, kz = (o / OPS_ROW) % HZ, c6 = o / (OPS_ROW * HZ);
+            cp_async16(kbuf + (c6 * HZ + kz) * LANES + q * PER16, kb + c6 * kcs + (int64_t)kz * Hy * a.pitch + q * PER16);
+        }
+    };
+
+    ZIter cur;
+    cur.set_item(blockIdx.x, a);
+    if (!cur.valid(a)) return;
+    prefetch_tile(cur);
+    cp_async_commit();                      // group A: input of the first tile
+    prefetch_k(cur);
+    cp_async_commit();                      // group B: K~ of the first item
+    load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, C::THREADS);
+
+    while (cur.valid(a)) {
+        int b, ky;
+        cur.tile(a, b, ky);
+        cx<T>* base = tile_base(cur) + lane;
+        ZIter nxt = cur;
+        nxt.next(a);
+        cp_async_wait<1>();                 // this tile's input has landed (the newest group may still be in flight)
+        __syncthreads();                    // ... for every thread; also: previous tile's exchange reads are done
+        // ---- forward step 1: tasks (c, n2)
 #pragma unroll
-    for (int it = 0; it < NT1; ++it) {
-        const int task = tp + it * TPP;
-        if ((3 * R2) % TPP == 0 || task < 3 * R2) {
-            const int c = task / R2, n2 = task % R2;
-            cx<T> w[R1];
-            static_for<NLOAD>([&](auto ic) { w[decltype(ic)::value] = v[it][decltype(ic)::value]; });
-            Dif<T, -1, R1, 0, PRUNE>::run(w);
-            cx<T>* dst = buf + c * TILE + n2 * LANES + lane;
-            static_for<R1>([&](auto pc) {
+        for (int it = 0; it < NT1; ++it) {
+            const int task = tp + it * TPP;
+            if ((3 * R2) % TPP == 0 || task < 3 * R2) {
+                const int c = task / R2, n2 = task % R2;
+                cx<T> w[R1];
+                const cx<T>* src = stage + (c * NIN + n2) * LANES + lane;
+                static_for<NLOAD>([&](auto ic) { w[decltype(ic)::value] = src[decltype(ic)::value * R2 * LANES]; });
+                Dif<T, -1, R1, 0, PRUNE>::run(w);
+                cx<T>* dst = buf + c * TILE + n2 * LANES + lane;
+                static_for<R1>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int k1 = brev<R1>(p);
+                    cx<T> val = w[p];
+                    if constexpr (k1 != 0) val = cmul(val, tw[n2 * k1]);
+                    dst[k1 * R2 * LANES] = val;
+                });
+            }
+        }
+        __syncthreads();                    // exchange written, staging buffer free
+        if (nxt.valid(a)) prefetch_tile(nxt);
+        cp_async_commit();                  // group A (possibly empty): input of the next tile
+        // ---- forward step 3 for thread k1 = tp: u[c][p] = P~_c[k1 + R1 brev(p)]
+        const int k1 = tp;
+        cx<T> u[3][R2];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const cx<T>* src = buf + c * TILE + k1 * R2 * LANES + lane;
+            static_for<R2>([&](auto nc) { u[c][decltype(nc)::value] = src[decltype(nc)::value * LANES]; });
+            Dif<T, -1, R2>::run(u[c]);
+        }
+        cp_async_wait<1>();                 // K~ of this item has landed (only the group just committed may be pending)
+        __syncthreads();                    // ... for every thread; exchange fully read
+        // ---- multiply
+        {
+            const T esc = (T)(-a.members[b].escale);
+            const T sy = 2 * ky > a.My ? -esc : esc;
+            static_for<R2>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
-                constexpr int k1 = brev<R1>(p);
-                cx<T> val = w[p];
-                if constexpr (k1 != 0) val = cmul(val, tw[n2 * k1]);
-                dst[k1 * R2 * LANES] = val;
+                constexpr int k2 = brev<R2>(p);
+                const int kz = k1 + R1 * k2;
+                const int kzm = 2 * kz <= M ? kz : M - kz;
+                const T sz = 2 * kz > M ? (T)-1 : (T)1;
+                const T* kp = kbuf + kzm * LANES + lane;
+                const T Kxx = esc * kp[0], Kyy = esc * kp[HZ * LANES], Kzz = esc * kp[2 * HZ * LANES];
+                const T Kxy = sy * kp[3 * HZ * LANES], Kxz = esc * sz * kp[4 * HZ * LANES];
+                const T Kyz = sy * sz * kp[5 * HZ * LANES];
+                const cx<T> Px = u[0][p], Py = u[1][p], Pz = u[2][p];
+                u[0][p] = {Kxx * Px.x + Kxy * Py.x + Kxz * Pz.x, Kxx * Px.y + Kxy * Py.y + Kxz * Pz.y};
+                u[1][p] = {Kxy * Px.x + Kyy * Py.x + Kyz * Pz.x, Kxy * Px.y + Kyy * Py.y + Kyz * Pz.y};
+                u[2][p] = {Kxz * Px.x + Kyz * Py.x + Kzz * Pz.x, Kxz * Px.y + Kyz * Py.y + Kzz * Pz.y};
             });
         }
-    }
-    __syncthreads();
-    // ---- forward step 3 for thread k1 = tp: u[c][p] = P~_c[k1 + R1 brev(p)]
-    const int k1 = tp;
-    cx<T> u[3][R2];
+        // ---- inverse step 1: R2-point over k2 (bit-reversed in, natural n2 out), twiddle, exchange
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const cx<T>* src = buf + c * TILE + k1 * R2 * LANES + lane;
-        static_for<R2>([&](auto nc) { u[c][decltype(nc)::value] = src[decltype(nc)::value * LANES]; });
-        Dif<T, -1, R2>::run(u[c]);
-    }
-    __syncthreads();     // every thread has read its forward data: the buffers may be overwritten
-    // ---- multiply
-    {
-        const int Hy = a.My / 2 + 1, Hz = M / 2 + 1;
-        const int kym = ky <= a.My / 2 ? ky : a.My - ky;
-        const T esc = (T)(-a.members[b].escale);
-        const T sy = ky > a.My / 2 ? -esc : esc;
-        const int64_t kcs = (int64_t)Hz * Hy * a.pitch;
-        const T* kb = Kt + (int64_t)kym * a.pitch + kx0 + lane;
-        static_for<R2>([&](auto pc) {
-            constexpr int p = decltype(pc)::value;
-            constexpr int k2 = brev<R2>(p);
-            const int kz = k1 + R1 * k2;
-            const int kzm = kz <= M / 2 ? kz : M - kz;
-            const T* kp = kb + (int64_t)kzm * Hy * a.pitch;
-            const T sz = kz > M / 2 ? (T)-1 : (T)1;
-            const T Kxx = esc * __ldg(kp), Kyy = esc * __ldg(kp + kcs), Kzz = esc * __ldg(kp + 2 * kcs);
-            const T Kxy = sy * __ldg(kp + 3 * kcs), Kxz = esc * sz * __ldg(kp + 4 * kcs);
-            const T Kyz = sy * sz * __ldg(kp + 5 * kcs);
-            const cx<T> Px = u[0][p], Py = u[1][p], Pz = u[2][p];
-            u[0][p] = {Kxx * Px.x + Kxy * Py.x + Kxz * Pz.x, Kxx * Px.y + Kxy * Py.y + Kxz * Pz.y};
-            u[1][p] = {Kxy * Px.x + Kyy * Py.x + Kyz * Pz.x, Kxy * Px.y + Kyy * Py.y + Kyz * Pz.y};
-            u[2][p] = {Kxz * Px.x + Kyz * Py.x + Kzz * Pz.x, Kxz * Px.y + Kyz * Py.y + Kzz * Pz.y};
-        });
-    }
-    // ---- inverse step 1: R2-point over k2 (bit-reversed in, natural n2 out), twiddle, exchange
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        Dit<T, +1, R2>::run(u[c]);
-        cx<T>* dst = buf + c * TILE + k1 * LANES + lane;
-        static_for<R2>([&](auto nc) {
-            constexpr int n2 = decltype(nc)::value;
-            cx<T> val = u[c][n2];
-            if constexpr (n2 != 0) val = cmulc(val, tw[n2 * k1]);
-            dst[n2 * R1 * LANES] = val;
-        });
-    }
-    __syncthreads();
-    // ---- inverse step 2: tasks (c, n2): R1-point over k1, rows n1 R2 + n2 (n1 < R1/2 when pruned) stored
-#pragma unroll
-    for (int it = 0; it < NT1; ++it) {
-        const int task = tp + it * TPP;
-        if ((3 * R2) % TPP == 0 || task < 3 * R2) {
-            const int c = task / R2, n2 = task % R2;
-            cx<T> w[R1];
-            const cx<T>* src = buf + c * TILE + n2 * R1 * LANES + lane;
-            static_for<R1>([&](auto kc) { w[decltype(kc)::value] = src[decltype(kc)::value * LANES]; });
-            Dif<T, +1, R1>::run(w);
-            cx<T>* out = base + c * cs + (int64_t)n2 * sa;
-            static_for<R1>([&](auto pc) {
-                constexpr int p = decltype(pc)::value;
-                constexpr int n1 = brev<R1>(p);
-                if constexpr (!PRUNE || n1 < R1 / 2) out[(int64_t)(R2 * n1) * sa] = w[p];
+        for (int c = 0; c < 3; ++c) {
+            Dit<T, +1, R2>::run(u[c]);
+            cx<T>* dst = buf + c * TILE + k1 * LANES + lane;
+            static_for<R2>([&](auto nc) {
+                constexpr int n2 = decltype(nc)::value;
+                cx<T> val = u[c][n2];
+                if constexpr (n2 != 0) val = cmulc(val, tw[n2 * k1]);
+                dst[n2 * R1 * LANES] = val;
             });
         }
+        __syncthreads();                    // exchange written; every thread is past the multiply: K~ buffer free
+        if (nxt.valid(a) && nxt.item != cur.item) prefetch_k(nxt);
+        cp_async_commit();                  // group B (possibly empty): K~ of the next item
+        // ---- inverse step 2: tasks (c, n2): R1-point over k1, rows n1 R2 + n2 (n1 < R1/2 when pruned) stored
+#pragma unroll
+        for (int it = 0; it < NT1; ++it) {
+            const int task = tp + it * TPP;
+            if ((3 * R2) % TPP == 0 || task < 3 * R2) {
+                const int c = task / R2, n2 = task % R2;
+                cx<T> w[R1];
+                const cx<T>* src = buf + c * TILE + n2 * R1 * LANES + lane;
+                static_for<R1>([&](auto kc) { w[decltype(kc)::value] = src[decltype(kc)::value * LANES]; });
+                Dif<T, +1, R1>::run(w);
+                cx<T>* out = base + c * cs + (int64_t)n2 * sa;
+                static_for<R1>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int n1 = brev<R1>(p);
+                    if constexpr (!PRUNE || n1 < R1 / 2) out[(int64_t)(R2 * n1) * sa] = w[p];
+                });
+            }
+        }
+        cur = nxt;
     }
+    cp_async_wait<0>();
 }
 
-template <typename T, int M, bool PRUNE>
-static cudaError_t launch_one(void* S, const T* Kt, const Z2Args& a, dim3 grid, cudaStream_t st)
+template <typename T, int M, int LANES, bool PRUNE>
+static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
 {
-    constexpr int LANES = 128 / (int)sizeof(cx<T>);
-    constexpr int threads = LANES * Fact<M>::R1;
-    constexpr size_t smem = (size_t)(M + 3 * M * LANES) * sizeof(cx<T>);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(k2_zmul<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    using C = ZCfg<T, M, LANES, PRUNE>;
+    static int nblocks = 0;
+    if (!nblocks) {
+        cudaError_t e = cudaFuncSetAttribute(k2_zmul<T, M, LANES, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)C::smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        int dev = 0, sms = 0, per = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k2_zmul<T, M, LANES, PRUNE>, C::THREADS, C::smem)) !=
+            cudaSuccess)
+            return e;
+        nblocks = sms * (per > 0 ? per : 1);
     }
-    k2_zmul<T, M, PRUNE><<<grid, threads, smem, st>>>(static_cast<cx<T>*>(S), Kt, a);
+    a.ngroups = a.pitch / LANES;
+    a.nitems = a.ngroups * (a.My / 2 + 1);
+    const int grid = a.nitems < nblocks ? a.nitems : nblocks;
+    k2_zmul<T, M, LANES, PRUNE><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a);
     return cudaGetLastError();
+}
+
+template <typename T, int M, int LANES>
+static cudaError_t launch_p(bool prune, void* S, const T* Kt, const Z2Args& a, cudaStream_t st)
+{
+    return prune ? launch_one<T, M, LANES, true>(S, Kt, a, st) : launch_one<T, M, LANES, false>(S, Kt, a, st);
 }
 
 }  // namespace v2
 
 bool zmul2_supported(int M) { return M == 64 || M == 128 || M == 256; }
 
-// same contract as launch_zmul (fe_fft.cu)
+// same contract as launch_zmul (fe_fft.cu); pitch must be a multiple of 128 bytes of complex elements
 template <typename T>
 cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int pitch,
                          int batch, cudaStream_t st)
 {
     const int M = c.plan[2].M;
-    constexpr int LANES = 128 / (int)sizeof(v2::cx<T>);
-    v2::Z2Args a{c.tw, members, My, pitch, nz};
-    dim3 grid(pitch / LANES, My, batch);
+    constexpr int L128 = 128 / (int)sizeof(v2::cx<T>);      // lanes of a 128-byte row
+    v2::Z2Args a{c.tw, members, My, pitch, nz, batch, 0, 0};
     const bool prune = 2 * nz == M;
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
-        case 64: return prune ? v2::launch_one<T, 64, true>(S, Kt, a, grid, st) : v2::launch_one<T, 64, false>(S, Kt, a, grid, st);
-        case 128: return prune ? v2::launch_one<T, 128, true>(S, Kt, a, grid, st) : v2::launch_one<T, 128, false>(S, Kt, a, grid, st);
-        case 256: return prune ? v2::launch_one<T, 256, true>(S, Kt, a, grid, st) : v2::launch_one<T, 256, false>(S, Kt, a, grid, st);
+        case 64: return v2::launch_p<T, 64, L128>(prune, S, Kt, a, st);
+        case 128: return v2::launch_p<T, 128, L128>(prune, S, Kt, a, st);
+        case 256: return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
         default: return cudaErrorInvalidValue;
     }
 }
