@@ -44,7 +44,12 @@ template <typename T, int M, int LANES, bool PRUNE> struct ZCfg {
     static constexpr int TPP = R1;                          // threads per pencil (one step-3 task each)
     static constexpr int THREADS = LANES * TPP;
     static constexpr int NT1 = (3 * R2 + TPP - 1) / TPP;    // step-1 tasks (component, n2) per thread
-    static constexpr int TILE = M * LANES;                  // exchange tile of one component (complex)
+    // exchange tile of one component: rows of LANES complex.  When a row is shorter than 128 bytes two threads
+    // of one shared-memory phase sit in rows R2 (forward) or R1 (inverse) apart; one pad row per group of R2 / R1
+    // rows shifts them into different bank halves.
+    static constexpr int PAD = LANES * (int)sizeof(cx<T>) < 128 ? 1 : 0;
+    static constexpr int P2 = R2 + PAD, P1 = R1 + PAD;      // row pitch of a k1 group (forward) / n2 group (inverse)
+    static constexpr int TILE = (R1 * P2 > R2 * P1 ? R1 * P2 : R2 * P1) * LANES;
     static constexpr int NIN = PRUNE ? M / 2 : M;           // input rows per component
     static constexpr int HZ = M / 2 + 1;
     static constexpr size_t tw_bytes = (size_t)M * sizeof(cx<T>);
@@ -86,6 +91,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
 {
     using C = ZCfg<T, M, LANES, PRUNE>;
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT1 = C::NT1, TILE = C::TILE, NIN = C::NIN, HZ = C::HZ;
+    constexpr int P1 = C::P1, P2 = C::P2;
     constexpr int NLOAD = PRUNE ? R1 / 2 : R1;
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);
     cx<T>* buf = tw + M;                                            // exchange [3][M][LANES]
@@ -134,6 +140,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         int b, ky;
         cur.tile(a, b, ky);
         cx<T>* base = tile_base(cur) + lane;
+        const double escale = a.members[b].escale;      // issued here, consumed after the forward transform
         ZIter nxt = cur;
         nxt.next(a);
         cp_async_wait<1>();                 // this tile's input has landed (the newest group may still be in flight)
@@ -154,7 +161,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                     constexpr int k1 = brev<R1>(p);
                     cx<T> val = w[p];
                     if constexpr (k1 != 0) val = cmul(val, tw[n2 * k1]);
-                    dst[k1 * R2 * LANES] = val;
+                    dst[k1 * P2 * LANES] = val;
                 });
             }
         }
@@ -166,7 +173,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         cx<T> u[3][R2];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const cx<T>* src = buf + c * TILE + k1 * R2 * LANES + lane;
+            const cx<T>* src = buf + c * TILE + k1 * P2 * LANES + lane;
             static_for<R2>([&](auto nc) { u[c][decltype(nc)::value] = src[decltype(nc)::value * LANES]; });
             Dif<T, -1, R2>::run(u[c]);
         }
@@ -174,7 +181,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         __syncthreads();                    // ... for every thread; exchange fully read
         // ---- multiply
         {
-            const T esc = (T)(-a.members[b].escale);
+            const T esc = (T)(-escale);
             const T sy = 2 * ky > a.My ? -esc : esc;
             static_for<R2>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
@@ -201,7 +208,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                 constexpr int n2 = decltype(nc)::value;
                 cx<T> val = u[c][n2];
                 if constexpr (n2 != 0) val = cmulc(val, tw[n2 * k1]);
-                dst[n2 * R1 * LANES] = val;
+                dst[n2 * P1 * LANES] = val;
             });
         }
         __syncthreads();                    // exchange written; every thread is past the multiply: K~ buffer free
@@ -214,7 +221,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
             if ((3 * R2) % TPP == 0 || task < 3 * R2) {
                 const int c = task / R2, n2 = task % R2;
                 cx<T> w[R1];
-                const cx<T>* src = buf + c * TILE + n2 * R1 * LANES + lane;
+                const cx<T>* src = buf + c * TILE + n2 * P1 * LANES + lane;
                 static_for<R1>([&](auto kc) { w[decltype(kc)::value] = src[decltype(kc)::value * LANES]; });
                 Dif<T, +1, R1>::run(w);
                 cx<T>* out = base + c * cs + (int64_t)n2 * sa;
