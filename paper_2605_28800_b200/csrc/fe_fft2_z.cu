@@ -13,6 +13,7 @@
 //   forward   x[n2 + R2 n1] -> (R1-point over n1) -> twiddle -> exchange -> (R2-point over n2) -> X[k1 + R1 k2]
 //   inverse   X[k1 + R1 k2] -> (R2-point over k2) -> twiddle -> exchange -> (R1-point over k1) -> x[n1 R2 + n2]
 #include "fe_fft2.cuh"
+#include <stdlib.h>
 
 namespace fe {
 namespace v2 {
@@ -35,6 +36,17 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(s), "l"(gmem));
+}
+// copy BYTES (8 or 16) bytes
+template <int BYTES> __device__ __forceinline__ void cp_async_n(void* smem, const void* gmem)
+{
+    if constexpr (BYTES == 16) cp_async16(smem, gmem);
+    else cp_async8(smem, gmem);
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
@@ -86,7 +98,7 @@ struct ZIter {
 };
 
 template <typename T, int M, int LANES, bool PRUNE>
-__global__ void __launch_bounds__(ZCfg<T, M, LANES, PRUNE>::THREADS, 2)
+__global__ void __launch_bounds__(ZCfg<T, M, LANES, PRUNE>::THREADS, ZCfg<T, M, LANES, PRUNE>::THREADS <= 64 ? 4 : 2)
 k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
 {
     using C = ZCfg<T, M, LANES, PRUNE>;
@@ -109,21 +121,37 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
     auto prefetch_tile = [&](const ZIter& it) {
-        const cx<T>* base = tile_base(it);
-        constexpr int PER16 = 16 / (int)sizeof(cx<T>);              // complex elements per 16-byte copy
-        constexpr int OPS_ROW = LANES / PER16, OPS = 3 * NIN * OPS_ROW;
-        for (int o = threadIdx.x; o < OPS; o += C::THREADS) {
-            const int q = o % OPS_ROW, row = (o / OPS_ROW) % NIN, c = o / (OPS_ROW * NIN);
-            cp_async16(stage + (c * NIN + row) * LANES + q * PER16, base + c * cs + (int64_t)row * sa + q * PER16);
+        constexpr int CB = LANES * (int)sizeof(cx<T>) < 16 ? 8 : 16;   // bytes per copy
+        constexpr int PER = CB / (int)sizeof(cx<T>);                    // complex elements per copy
+        constexpr int OPS_ROW = LANES / PER;                            // copies per row
+        constexpr int RSTEP = C::THREADS / OPS_ROW;                     // rows covered by one sweep of the block
+        static_assert(C::THREADS % OPS_ROW == 0 && NIN % RSTEP == 0, "tile copy must be regular");
+        const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
+        const cx<T>* g = tile_base(it) + (int64_t)row0 * sa + q * PER;
+        cx<T>* s = stage + row0 * LANES + q * PER;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+#pragma unroll
+            for (int j = 0; j < NIN / RSTEP; ++j)
+                cp_async_n<CB>(s + (c * NIN + j * RSTEP) * LANES, g + c * cs + (int64_t)(j * RSTEP) * sa);
         }
     };
     auto prefetch_k = [&](const ZIter& it) {
-        constexpr int PER16 = 16 / (int)sizeof(T);
-        constexpr int OPS_ROW = LANES / PER16, OPS = 6 * HZ * OPS_ROW;
-        const T* kb = Kt + (int64_t)it.kyh * a.pitch + it.kxg * LANES;
-        for (int o = threadIdx.x; o < OPS; o += C::THREADS) {
-            const int q = o % OPS_ROW, kz = (o / OPS_ROW) % HZ, c6 = o / (OPS_ROW * HZ);
-            cp_async16(kbuf + (c6 * HZ + kz) * LANES + q * PER16, kb + c6 * kcs + (int64_t)kz * Hy * a.pitch + q * PER16);
+        constexpr int CB = LANES * (int)sizeof(T) < 16 ? 8 : 16;
+        constexpr int PER = CB / (int)sizeof(T);
+        constexpr int OPS_ROW = LANES / PER;
+        constexpr int RSTEP = C::THREADS / OPS_ROW;
+        static_assert(LANES * sizeof(T) >= 8 && C::THREADS % OPS_ROW == 0, "a K~ row of a tile must be at least 8 bytes");
+        const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
+        const int64_t krs = (int64_t)Hy * a.pitch;                      // stride of kz in the table
+        const T* g = Kt + (int64_t)it.kyh * a.pitch + it.kxg * LANES + (int64_t)row0 * krs + q * PER;
+        T* s = kbuf + row0 * LANES + q * PER;
+#pragma unroll
+        for (int c6 = 0; c6 < 6; ++c6) {
+#pragma unroll
+            for (int j = 0; j < (HZ + RSTEP - 1) / RSTEP; ++j)
+                if ((j + 1) * RSTEP <= HZ || row0 + j * RSTEP < HZ)
+                    cp_async_n<CB>(s + (c6 * HZ + j * RSTEP) * LANES, g + c6 * kcs + (int64_t)(j * RSTEP) * krs);
         }
     };
 
@@ -284,7 +312,11 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
     switch (M) {
         case 64: return v2::launch_p<T, 64, L128>(prune, S, Kt, a, st);
         case 128: return v2::launch_p<T, 128, L128>(prune, S, Kt, a, st);
-        case 256: return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
+        case 256: {
+            static const int zl = getenv("FE_B200_ZLANES") ? atoi(getenv("FE_B200_ZLANES")) : 0;   // tuning aid
+            if (zl == 2 && sizeof(T) == 8) return v2::launch_p<T, 256, 2>(prune, S, Kt, a, st);
+            return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
+        }
         default: return cudaErrorInvalidValue;
     }
 }

@@ -38,6 +38,38 @@ template <typename T> struct LandauT {
     }
 };
 
+// Coefficients of -E_Land,i / P_i = d f_Land / d P_i / P_i (Eq. 3) with the integer factors folded in:
+//   k1_i + k11 a + k12 (b+c) + k111 a^2 + k112 [2 a (b+c) + b^2 + c^2] + k123 b c
+//   + k1111 a^3 + k1112 [3 a^2 (b+c) + b^3 + c^3] + k1122 a (b^2+c^2) + k1123 b c (2 a + b + c)
+// with (a, b, c) = (P_i^2, the other two squared).
+template <typename T> struct LandauD {
+    T k1x, k1y, k1z, k11, k12, k111, k112, k123, k1111, k1112, k1122, k1123;
+    int o8;       // any 8th-order slot non-zero
+    int active;
+    __device__ LandauD() {}
+    __device__ explicit LandauD(const DevLandau& m)
+        : k1x((T)(2 * m.a1[0])), k1y((T)(2 * m.a1[1])), k1z((T)(2 * m.a1[2])), k11((T)(4 * m.a11)), k12((T)(2 * m.a12)),
+          k111((T)(6 * m.a111)), k112((T)(2 * m.a112)), k123((T)(2 * m.a123)), k1111((T)(8 * m.a1111)),
+          k1112((T)(2 * m.a1112)), k1122((T)(4 * m.a1122)), k1123((T)(2 * m.a1123)),
+          o8(m.a1111 != 0.0 || m.a1112 != 0.0 || m.a1122 != 0.0 || m.a1123 != 0.0), active(m.active != 0) {}
+    // a2 = a^2, b2c2 = b^2 + c^2, bc = b + c, bxc = b c
+    __device__ __forceinline__ T dfd(T k1i, T a, T a2, T bc, T b2c2, T bxc, T b3c3) const
+    {
+        T s = k1i + k11 * a;
+        s += k12 * bc;
+        s += k111 * a2;
+        s += k112 * ((a + a) * bc + b2c2);
+        s += k123 * bxc;
+        if (o8) {
+            s += k1111 * (a2 * a);
+            s += k1112 * ((T)3 * a2 * bc + b3c3);
+            s += k1122 * (a * b2c2);
+            s += k1123 * (bxc * (a + a + bc));
+        }
+        return s;
+    }
+};
+
 // neighbour coordinate along one axis; returns -1 if it falls outside an open axis
 __device__ __forceinline__ int nb(int c, int s, int n, int per)
 {
@@ -82,12 +114,12 @@ constexpr int kTX = 32, kTY = 8, kHX = kTX + 2, kHY = kTY + 2, kTile = kHX * kHY
 constexpr int kNL = (3 * kTile + 255) / 256;                                        // loader entries per thread
 
 template <typename T, bool MAP, bool MIXED>
-__global__ void __launch_bounds__(256) k_local(LocalArgs a)
+__global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
 {
     extern __shared__ __align__(16) unsigned char lsm[];
     T* tiles = reinterpret_cast<T*>(lsm);                                   // [4][3][kTile]
     unsigned char* flags = lsm + (size_t)4 * 3 * kTile * sizeof(T);         // [4][kTile]
-    LandauT<T>* smats = reinterpret_cast<LandauT<T>*>(flags + 4 * kTile + 8);  // [nmat]  (offset is 16-aligned)
+    LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + 4 * kTile + 8);  // [nmat]  (offset is 8-aligned)
     unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
 
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
@@ -100,18 +132,20 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
     const T* Y = static_cast<const T*>(a.Y) + (int64_t)b * 3 * N;
     const DevLandau* mats = a.mats + (int64_t)b * a.nmat;
     for (int m = t; m < a.nmat; m += 256) {
-        smats[m] = LandauT<T>(mats[m]);
+        smats[m] = LandauD<T>(mats[m]);
         sact[m] = mats[m].active != 0;
     }
     const DevMember mem = a.members[b];
 
     // loader entries: shared offset, in-plane global offset (-1: outside an open axis), component
     int l_so[kNL], l_go[kNL];
+    const T* l_ptr[kNL];
 #pragma unroll
     for (int k = 0; k < kNL; ++k) {
         const int idx = t + 256 * k;
         l_so[k] = -1;
         l_go[k] = -1;
+        l_ptr[k] = Y;
         if (idx < 3 * kTile) {
             const int rem = idx % kTile, yy = rem / kHX, xx = rem % kHX;
             int gx = x0 - 1 + xx, gy = y0 - 1 + yy;
@@ -120,6 +154,7 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
             if (gy < 0 || gy >= ny) { if (a.periodic[1]) gy = ((gy % ny) + ny) % ny; else in = false; }
             l_so[k] = idx;
             l_go[k] = in ? gy * nx + gx : -1;
+            if (in) l_ptr[k] = Y + (int64_t)(idx / kTile) * N + l_go[k];
         }
     }
     // global -> registers (issued one plane ahead of its use), registers -> shared tile
@@ -129,13 +164,13 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
         int zz = z;
         bool zin = true;
         if (zz < 0 || zz >= nz) { if (a.periodic[2]) zz = ((zz % nz) + nz) % nz; else zin = false; }
+        const int64_t r0 = (int64_t)zz * nxy;
 #pragma unroll
         for (int k = 0; k < kNL; ++k) {
             const bool ok = zin && l_go[k] >= 0;
-            const int64_t r = (int64_t)zz * nxy + l_go[k];
-            pre[k] = ok ? Y[(l_so[k] / kTile) * N + r] : (T)0;
+            pre[k] = ok ? l_ptr[k][r0] : (T)0;
             pok[k] = ok;
-            if (MAP) { if (ok) pok[k] = sact[a.map[r]] != 0; }
+            if (MAP) { if (ok) pok[k] = sact[a.map[r0 + l_go[k]]] != 0; }
         }
     };
     auto store_plane = [&](int z) {
@@ -146,7 +181,7 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
         for (int k = 0; k < kNL; ++k) {
             if (l_so[k] < 0) continue;
             tl[l_so[k]] = pok[k] ? pre[k] : (T)0;
-            if (l_so[k] < kTile) fl[l_so[k]] = pok[k];
+            if (MAP && l_so[k] < kTile) fl[l_so[k]] = pok[k];
         }
     };
     __syncthreads();          // coefficient tables visible (fetch_plane reads sact)
@@ -160,6 +195,9 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
     const bool inside = x < nx && y < ny;
     const int64_t rxy = (int64_t)y * nx + x;
     const int c0 = (ty + 1) * kHX + tx + 1;
+    // without a material map the existence of a neighbour is pure geometry
+    const T gxf = (T)((x > 0 || a.periodic[0]) + (x < nx - 1 || a.periodic[0]));
+    const T gyf = (T)((y > 0 || a.periodic[1]) + (y < ny - 1 || a.periodic[1]));
     const T G11 = (T)mem.G11, Gt = (T)mem.Gt, Gm = (T)mem.Gm, L = (T)mem.L;
     const T ix = (T)a.id2[0], iy = (T)a.id2[1], iz = (T)a.id2[2];
     const T qxy = Gm * (T)a.i4[0], qxz = Gm * (T)a.i4[1], qyz = Gm * (T)a.i4[2];
@@ -171,7 +209,7 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
     T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
     const T* ai = a.accOut ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
     T* ao = a.accOut ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
-    LandauT<T> lc0 = smats[0];
+    const LandauD<T> lc0 = smats[0];
 
     T en[3] = {0, 0, 0};
     if (Ee && inside) {
@@ -196,20 +234,25 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
         const unsigned char* fp = flags + ((z + 1) & 3) * kTile;
         const int64_t r = (int64_t)z * nxy + rxy;
         T k[3] = {0, 0, 0};
-        if (fc[c0]) {
+        if (!MAP || fc[c0]) {
             const T px = c[c0], py = c[kTile + c0], pz = c[2 * kTile + c0];
             T E0 = 0, E1 = 0, E2 = 0;
             if (a.terms & 1u) {
-                const LandauT<T> lc = MAP ? smats[a.map[r]] : lc0;
+                const LandauD<T> lc = MAP ? smats[a.map[r]] : lc0;
                 const T A = px * px, B = py * py, C = pz * pz;
-                E0 -= px * lc.dfd(lc.a1x, A, B, C);
-                E1 -= py * lc.dfd(lc.a1y, B, C, A);
-                E2 -= pz * lc.dfd(lc.a1z, C, A, B);
+                const T A2 = A * A, B2 = B * B, C2 = C * C;
+                T A3 = 0, B3 = 0, C3 = 0;
+                if (lc.o8) { A3 = A2 * A; B3 = B2 * B; C3 = C2 * C; }
+                E0 -= px * lc.dfd(lc.k1x, A, A2, B + C, B2 + C2, B * C, B3 + C3);
+                E1 -= py * lc.dfd(lc.k1y, B, B2, C + A, C2 + A2, C * A, C3 + A3);
+                E2 -= pz * lc.dfd(lc.k1z, C, C2, A + B, A2 + B2, A * B, A3 + B3);
             }
             if (a.terms & 2u) {
                 // bonds: sum over existing neighbours of c_ia / D_a^2 (P_i(nb) - P_i(r)); a missing neighbour holds 0
-                const T nxf = (T)(fc[c0 - 1] + fc[c0 + 1]), nyf = (T)(fc[c0 - kHX] + fc[c0 + kHX]);
-                const T nzf = (T)(fm[c0] + fp[c0]);
+                const T nxf = MAP ? (T)(fc[c0 - 1] + fc[c0 + 1]) : gxf;
+                const T nyf = MAP ? (T)(fc[c0 - kHX] + fc[c0 + kHX]) : gyf;
+                const T nzf = MAP ? (T)(fm[c0] + fp[c0])
+                                  : (T)((z > 0 || a.periodic[2]) + (z < nz - 1 || a.periodic[2]));
 #pragma unroll
                 for (int i = 0; i < 3; ++i) {
                     const T* ci = c + i * kTile;
@@ -244,7 +287,7 @@ __global__ void __launch_bounds__(256) k_local(LocalArgs a)
         if (base) {
             if (base_is_Y) {
                 // the stage base is the state itself (Euler): take it from the tile; vacuum cells hold their raw value
-                if (fc[c0]) { bv[0] = c[c0]; bv[1] = c[kTile + c0]; bv[2] = c[2 * kTile + c0]; }
+                if (!MAP || fc[c0]) { bv[0] = c[c0]; bv[1] = c[kTile + c0]; bv[2] = c[2 * kTile + c0]; }
                 else { bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r]; }
             } else {
                 bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r];
@@ -272,7 +315,7 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
     a.zchunk = zc;
     dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
-    const size_t smem = (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauT<T>) + 1);
+    const size_t smem = (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
     static bool configured = false;
     if (!configured) {
         const int lim = 96 * 1024;      // 255 materials need 61 KB
