@@ -98,7 +98,7 @@ struct ZIter {
 };
 
 template <typename T, int M, int LANES, bool PRUNE>
-__global__ void __launch_bounds__(ZCfg<T, M, LANES, PRUNE>::THREADS, ZCfg<T, M, LANES, PRUNE>::THREADS <= 64 ? 4 : 2)
+__global__ void __launch_bounds__(ZCfg<T, M, LANES, PRUNE>::THREADS, ZCfg<T, M, LANES, PRUNE>::THREADS <= 64 ? 4 : (ZCfg<T, M, LANES, PRUNE>::smem > 112 * 1024 ? 1 : 2))
 k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
 {
     using C = ZCfg<T, M, LANES, PRUNE>;
@@ -313,9 +313,11 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
         case 64: return v2::launch_p<T, 64, L128>(prune, S, Kt, a, st);
         case 128: return v2::launch_p<T, 128, L128>(prune, S, Kt, a, st);
         case 256: {
-            static const int zl = getenv("FE_B200_ZLANES") ? atoi(getenv("FE_B200_ZLANES")) : 0;   // tuning aid
-            if (zl == 2 && sizeof(T) == 8) return v2::launch_p<T, 256, 2>(prune, S, Kt, a, st);
-            return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
+            // 128-byte rows (one 256-thread block per SM) beat 64-byte rows (two 128-thread blocks) on B200:
+            // 0.66 vs 0.80 ms at cfg5a.  FE_B200_ZLANES=4 selects the narrow tile (tuning aid).
+            static const int zl = getenv("FE_B200_ZLANES") ? atoi(getenv("FE_B200_ZLANES")) : 0;
+            if (zl == 4 || sizeof(T) != 8) return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
+            return v2::launch_p<T, 256, L128>(prune, S, Kt, a, st);
         }
         default: return cudaErrorInvalidValue;
     }
