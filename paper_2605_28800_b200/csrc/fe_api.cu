@@ -62,6 +62,7 @@ struct fe_grid {
     int nblk;
     bool tensor_ready;
     bool fast[3];                    // size-specialised register FFT kernels available for the x / y / z pass
+    bool tiled;                      // spectra and tensor table in the tiled layouts (all three passes fast)
     uint64_t launches;
     // optional per-kernel CUDA-event timing (fe_profile): event i precedes the launch of kind prof_kind[i]
     bool prof_on;
@@ -213,6 +214,13 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
         g->fast[0] = !generic && x2_supported(q.m[0] / 2);
         g->fast[1] = !generic && axis2_supported(q.m[1]) && (size_t)q.lanes == lanes_full;
         g->fast[2] = !generic && zmul2_supported(q.m[2]) && (size_t)q.lanes == lanes_full;
+        // Tiled layouts (L = 128 bytes of consecutive kx, G = pitch / L groups), used when every pass is fast:
+        //   S1[b][c][z][g][y][L]   the y pass reads / writes whole contiguous tiles,
+        //   S2[b][c][g][ky][z][L]  the fused z pass works on contiguous tiles (no 2 MB strides),
+        //   Kt[6][g][ky][kz][L]    its tensor tile is contiguous too.
+        // FE_B200_LINEAR=1 keeps the row-major layouts (tuning aid).
+        const char* lin = getenv("FE_B200_LINEAR");
+        g->tiled = g->fast[0] && g->fast[1] && g->fast[2] && !(lin && lin[0] == '1');
     }
     g->dirty = true;
     g->mixed = 0;
@@ -423,8 +431,13 @@ static fe_status precompute_T(fe_grid* g, cudaStream_t st)
                                     p64 * q.m[1], 0, p64, p64 * q.m[1], 0, st));
         FE_CUDA(launch_axis<double>(g->ctx64, 2, -1, Sbox, Sbox, q.m[2], q.lanes64, q.pitch64, q.m[1], 1,
                                     p64 * q.m[1], p64, 0, p64 * q.m[1], p64, 0, st));
-        FE_CUDA(launch_extract<T>(Sbox, Kt + (int64_t)c * Hz * Hy * q.pitch, q.m[2], q.m[1], q.Lx, q.pitch64, q.pitch,
-                                  scale, st));
+        const int L = (int)(128 / g->csz);
+        if (g->tiled)
+            FE_CUDA(launch_extract<T>(Sbox, Kt + (int64_t)c * Hz * Hy * q.pitch, q.m[2], q.m[1], q.Lx, q.pitch64, q.pitch,
+                                      scale, L, L, (int64_t)Hz * L, (int64_t)Hy * Hz * L, st));
+        else
+            FE_CUDA(launch_extract<T>(Sbox, Kt + (int64_t)c * Hz * Hy * q.pitch, q.m[2], q.m[1], q.Lx, q.pitch64, q.pitch,
+                                      scale, L, (int64_t)Hy * q.pitch, q.pitch, L, st));
         g->launches += 5 + ((q.zero_mode && q.periodic[0] + q.periodic[1] + q.periodic[2] == 2) ? 1 : 0);
     }
     return FE_OK;
@@ -474,28 +487,47 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     const int64_t p = q.pitch;
     const int slabs = B * 3 * q.n[2];
     const int64_t rows = (int64_t)slabs * q.n[1];
+    const int L = (int)(128 / g->csz), G = q.pitch / L;
+    const int nx = q.n[0], ny = q.n[1], nz = q.n[2], My = q.m[1];
+    const int Hy = My / 2 + 1, Hz = q.m[2] / 2 + 1;
+    const bool tl = g->tiled;
+    // strides (complex elements; the tensor table in reals), row-major or tiled (see fe_create_grid)
+    const int64_t xspec[4] = {ny, p * ny, tl ? L : p, tl ? (int64_t)ny * L : L};             // S1 as the x passes see it
+    const int64_t y1_sa = tl ? L : p, y1_sg = tl ? (int64_t)ny * L : L, y1_sz = p * ny, y1_sb = p * ny * nz;   // S1, y pass
+    const int64_t y2_sa = tl ? (int64_t)nz * L : p, y2_sg = tl ? (int64_t)My * nz * L : L, y2_sz = tl ? L : p * My,
+                  y2_sb = p * My * nz;                                                          // S2, y pass
+    const int64_t zs[4] = {p * My * nz, tl ? L : p * My, tl ? (int64_t)nz * L : p, tl ? (int64_t)My * nz * L : L};
+    const int64_t ks[4] = {(int64_t)Hz * Hy * p, tl ? L : (int64_t)Hy * p, tl ? (int64_t)Hz * L : p,
+                           tl ? (int64_t)Hy * Hz * L : L};
     mark(g, K_XFWD, st);
-    if (g->fast[0]) FE_CUDA(launch_xfwd2<T>(g->ctx, Y, S1, q.n[0], rows, q.n[0], p, st));
+    if (g->fast[0]) FE_CUDA(launch_xfwd2<T>(g->ctx, Y, S1, nx, rows, nx, xspec, L, st));
     else FE_CUDA(launch_xfwd<T>(g->ctx, Y, S1, q.n[0], q.n[1], slabs, q.n[0], (int64_t)q.n[0] * q.n[1], p, p * q.n[1], st));
     mark(g, K_YFWD, st);
-    if (g->fast[1])
-        FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.pitch, q.n[2], B * 3, p, p * q.n[1],
-                                p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
-    else
+    if (g->fast[1]) {
+        // tiled: z is the fastest block index, so that concurrently running blocks write neighbouring 128-byte pieces
+        if (tl) FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, ny, nz, G, B * 3, y1_sa, y1_sz, y1_sg, y1_sb,
+                                        y2_sa, y2_sz, y2_sg, y2_sb, st));
+        else FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, ny, G, nz, B * 3, y1_sa, y1_sg, y1_sz, y1_sb,
+                                     y2_sa, y2_sg, y2_sz, y2_sb, st));
+    } else {
         FE_CUDA(launch_axis<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.n[1],
                                p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
+    }
     mark(g, K_ZMUL, st);
-    if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.pitch, B, st));
+    if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, st));
     else FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
     mark(g, K_YINV, st);
-    if (g->fast[1])
-        FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.pitch, q.n[2], B * 3, p, p * q.m[1],
-                                p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
-    else
+    if (g->fast[1]) {
+        if (tl) FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, ny, nz, G, B * 3, y2_sa, y2_sz, y2_sg, y2_sb,
+                                        y1_sa, y1_sz, y1_sg, y1_sb, st));
+        else FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, ny, G, nz, B * 3, y2_sa, y2_sg, y2_sz, y2_sb,
+                                     y1_sa, y1_sg, y1_sz, y1_sb, st));
+    } else {
         FE_CUDA(launch_axis<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.m[1],
                                p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
+    }
     mark(g, K_XINV, st);
-    if (g->fast[0]) FE_CUDA(launch_xinv2<T>(g->ctx, S1, E, q.n[0], rows, p, q.n[0], st));
+    if (g->fast[0]) FE_CUDA(launch_xinv2<T>(g->ctx, S1, E, nx, rows, nx, xspec, L, st));
     else FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
     g->launches += 5;
     return FE_OK;

@@ -363,16 +363,18 @@ __global__ void __launch_bounds__(kThreads) k_zmul(cx<T>* __restrict__ S, const 
     }
 }
 
-// complex fp64 spectrum of one tensor component on the box -> real table for kz <= Mz/2, ky <= My/2
+// complex fp64 spectrum of one tensor component on the box -> real table for kz <= Mz/2, ky <= My/2.
+// Entry (kz, ky, kx) is written at kz * k_skz + ky * k_sky + (kx >> lg) * k_sg + (kx & (2^lg - 1)): row-major
+// (k_skz = Hy pitch, k_sky = pitch, k_sg = 2^lg) or the tiled layout of fe_api.cu.
 template <typename T>
-__global__ void k_extract(const cx<double>* __restrict__ Sbox, T* __restrict__ Kt, int Hz, int Hy, int My, int Lx,
-                          int pitch64, int pitchT, double scale)
+__global__ void k_extract(const cx<double>* __restrict__ Sbox, T* __restrict__ Kt, int My, int Lx, int pitch64,
+                          int pitchT, double scale, int lg, int64_t k_skz, int64_t k_sky, int64_t k_sg)
 {
     const int kz = blockIdx.z, ky = blockIdx.y;
     for (int kx = blockIdx.x * blockDim.x + threadIdx.x; kx < pitchT; kx += gridDim.x * blockDim.x) {
         double v = 0.0;
         if (kx < Lx) v = Sbox[((int64_t)kz * My + ky) * pitch64 + kx].x * scale;
-        Kt[((int64_t)kz * Hy + ky) * pitchT + kx] = (T)v;
+        Kt[(int64_t)kz * k_skz + (int64_t)ky * k_sky + (int64_t)(kx >> lg) * k_sg + (kx & ((1 << lg) - 1))] = (T)v;
     }
 }
 
@@ -438,12 +440,14 @@ cudaError_t launch_zmul(const FftCtx& c, void* S, const T* Kt, const DevMember* 
 
 template <typename T>
 cudaError_t launch_extract(const void* Sbox, T* Kt_comp, int Mz, int My, int Lx, int pitch64, int pitchT,
-                           double scale, cudaStream_t st)
+                           double scale, int lanes, int64_t k_skz, int64_t k_sky, int64_t k_sg, cudaStream_t st)
 {
     const int Hz = Mz / 2 + 1, Hy = My / 2 + 1;
+    int lg = 0;
+    while ((1 << lg) < lanes) ++lg;
     dim3 grid((pitchT + 127) / 128, Hy, Hz);
-    k_extract<T><<<grid, 128, 0, st>>>(static_cast<const cx<double>*>(Sbox), Kt_comp, Hz, Hy, My, Lx, pitch64,
-                                       pitchT, scale);
+    k_extract<T><<<grid, 128, 0, st>>>(static_cast<const cx<double>*>(Sbox), Kt_comp, My, Lx, pitch64, pitchT, scale,
+                                       lg, k_skz, k_sky, k_sg);
     return cudaGetLastError();
 }
 
@@ -470,7 +474,8 @@ cudaError_t fft_configure()
                                         int64_t, int64_t, int64_t, int64_t, int64_t, int64_t, cudaStream_t);       \
     template cudaError_t launch_zmul<T>(const FftCtx&, void*, const T*, const DevMember*, int, int, int, int, int, \
                                         cudaStream_t);                                                             \
-    template cudaError_t launch_extract<T>(const void*, T*, int, int, int, int, int, double, cudaStream_t);
+    template cudaError_t launch_extract<T>(const void*, T*, int, int, int, int, int, double, int, int64_t, int64_t,   \
+                                           int64_t, cudaStream_t);
 FE_INST(double)
 FE_INST(float)
 

@@ -10,11 +10,18 @@
 namespace fe {
 namespace v2 {
 
+// Real row r starts at r * real_rs.  Spectrum element k of row r sits at
+// (r / ny) * s_plane + (r % ny) * s_row + (k >> lg) * s_g + (k & (2^lg - 1))   (complex elements; 2^lg = kx per group),
+// which covers the row-major spectra (s_g = 2^lg) and the tiled layout of fe_api.cu.
 struct X2Args {
     const void* tw;
     int64_t nrows;
-    int64_t real_rs, spec_rs;     // row strides in reals / complex elements
+    int64_t real_rs;
+    int ny, lg;
+    int64_t s_plane, s_row, s_g;
 };
+__device__ __forceinline__ int64_t spec_off(const X2Args& a, int k) { return (int64_t)(k >> a.lg) * a.s_g + (k & ((1 << a.lg) - 1)); }
+__device__ __forceinline__ int64_t spec_row(const X2Args& a, int64_t row) { return (row / a.ny) * a.s_plane + (row % a.ny) * a.s_row; }
 
 template <int M> struct XCfg {
     static constexpr int R1 = Fact<M>::R1, R2 = Fact<M>::R2;
@@ -47,8 +54,9 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
     }
     {
         const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
+        // tw[k1 * R2 + n2] = w_M^(n2 k1): the R2 threads of a row read consecutive entries (no bank conflicts)
         for (int e = threadIdx.x; e < M; e += 256) {
-            tw[e] = twg[e * (kTwiddleN / M)];
+            tw[e] = twg[((e / R2) * (e % R2)) * (kTwiddleN / M)];
             tws[e] = twg[e * (kTwiddleN / (2 * M))];
         }
     }
@@ -58,7 +66,7 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
         constexpr int p = decltype(pc)::value;
         constexpr int k1 = brev<R1>(p);
         cx<T> val = v[p];
-        if constexpr (k1 != 0) val = cmul(val, tw[tp * k1]);
+        if constexpr (k1 != 0) val = cmul(val, tw[k1 * R2 + tp]);
         rb[k1 * (R2 + 1) + tp] = val;
     });
     __syncthreads();
@@ -80,7 +88,7 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
     }
     __syncthreads();
     if (live) {
-        cx<T>* dst = out + row * a.spec_rs;
+        cx<T>* dst = out + spec_row(a, row);
         for (int k = tp; k <= M / 2; k += TPP) {
             const cx<T> Zk = rb[k], Zn = rb[(M - k) & (M - 1)];
             const T ex = (T)0.5 * (Zk.x + Zn.x), ey = (T)0.5 * (Zk.y - Zn.y);
@@ -88,8 +96,8 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
             const cx<T> w = tws[k];
             // X[k] = Xe + w Xo;  X[M-k] = conj(Xe) - conj(w Xo)   (w_2M^(M-k) = -conj(w_2M^k), Xo(M-k) = conj Xo(k))
             const T px = ox * w.x - oy * w.y, py = ox * w.y + oy * w.x;
-            dst[k] = {ex + px, ey + py};
-            dst[M - k] = {ex - px, py - ey};
+            dst[spec_off(a, k)] = {ex + px, ey + py};
+            dst[spec_off(a, M - k)] = {ex - px, py - ey};
         }
     }
 }
@@ -109,18 +117,19 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
 
     {
         const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
+        // tw[k1 * R2 + n2] = w_M^(n2 k1): the R2 threads of a row read consecutive entries (no bank conflicts)
         for (int e = threadIdx.x; e < M; e += 256) {
-            tw[e] = twg[e * (kTwiddleN / M)];
+            tw[e] = twg[((e / R2) * (e % R2)) * (kTwiddleN / M)];
             tws[e] = twg[e * (kTwiddleN / (2 * M))];
         }
     }
     __syncthreads();
     cx<T> v[R1];
-    const cx<T>* src = in + (live ? row : 0) * a.spec_rs;
+    const cx<T>* src = in + spec_row(a, live ? row : 0);
     static_for<R1>([&](auto jc) {
         constexpr int j1 = decltype(jc)::value;
         const int k = tp + R2 * j1;
-        const cx<T> Xk = src[k], Xn = src[M - k];
+        const cx<T> Xk = src[spec_off(a, k)], Xn = src[spec_off(a, M - k)];
         const T ex = (T)0.5 * (Xk.x + Xn.x), ey = (T)0.5 * (Xk.y - Xn.y);
         const T dx = (T)0.5 * (Xk.x - Xn.x), dy = (T)0.5 * (Xk.y + Xn.y);
         const cx<T> w = tws[k];
@@ -132,7 +141,7 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
         constexpr int p = decltype(pc)::value;
         constexpr int o1 = brev<R1>(p);
         cx<T> val = v[p];
-        if constexpr (o1 != 0) val = cmulc(val, tw[tp * o1]);
+        if constexpr (o1 != 0) val = cmulc(val, tw[o1 * R2 + tp]);
         rb[o1 * (R2 + 1) + tp] = val;
     });
     __syncthreads();
@@ -194,32 +203,37 @@ static cudaError_t launch_x(int M, bool prune, const void* in, void* out, const 
 
 bool x2_supported(int Mc) { return Mc == 64 || Mc == 128 || Mc == 256 || Mc == 512; }
 
-// nrows uniformly strided rows: n_real valid reals per row (n_real == 2 Mc, or Mc when zero-padded)
+// nrows real rows of n_real valid reals (n_real == 2 Mc, or Mc when zero-padded), real_rs apart; spectrum strides
+// spec[4] = { ny (rows per plane), s_plane, s_row, s_g } as in X2Args, lanes = kx per group (power of two)
 template <typename T>
 cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, int64_t nrows, int64_t real_rs,
-                         int64_t spec_rs, cudaStream_t st)
+                         const int64_t spec[4], int lanes, cudaStream_t st)
 {
     const int M = c.plan[0].M;
     const bool prune = n_real == M;
     if (!prune && n_real != 2 * M) return cudaErrorInvalidValue;
-    v2::X2Args a{c.tw, nrows, real_rs, spec_rs};
+    int lg = 0;
+    while ((1 << lg) < lanes) ++lg;
+    v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3]};
     return v2::launch_x<T, true>(M, prune, in, out, a, st);
 }
 
 template <typename T>
-cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t spec_rs,
-                         int64_t real_rs, cudaStream_t st)
+cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t real_rs,
+                         const int64_t spec[4], int lanes, cudaStream_t st)
 {
     const int M = c.plan[0].M;
     const bool prune = n_real == M;
     if (!prune && n_real != 2 * M) return cudaErrorInvalidValue;
-    v2::X2Args a{c.tw, nrows, real_rs, spec_rs};
+    int lg = 0;
+    while ((1 << lg) < lanes) ++lg;
+    v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3]};
     return v2::launch_x<T, false>(M, prune, in, out, a, st);
 }
 
-template cudaError_t launch_xfwd2<double>(const FftCtx&, const double*, void*, int, int64_t, int64_t, int64_t, cudaStream_t);
-template cudaError_t launch_xfwd2<float>(const FftCtx&, const float*, void*, int, int64_t, int64_t, int64_t, cudaStream_t);
-template cudaError_t launch_xinv2<double>(const FftCtx&, const void*, double*, int, int64_t, int64_t, int64_t, cudaStream_t);
-template cudaError_t launch_xinv2<float>(const FftCtx&, const void*, float*, int, int64_t, int64_t, int64_t, cudaStream_t);
+template cudaError_t launch_xfwd2<double>(const FftCtx&, const double*, void*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);
+template cudaError_t launch_xfwd2<float>(const FftCtx&, const float*, void*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);
+template cudaError_t launch_xinv2<double>(const FftCtx&, const void*, double*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);
+template cudaError_t launch_xinv2<float>(const FftCtx&, const void*, float*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);
 
 }  // namespace fe

@@ -24,12 +24,17 @@ template <> struct ZFact<64> { static constexpr int R1 = 8, R2 = 8; };
 template <> struct ZFact<128> { static constexpr int R1 = 16, R2 = 8; };
 template <> struct ZFact<256> { static constexpr int R1 = 32, R2 = 8; };
 
+// Spectrum element (b, c, z, ky, kx) sits at b * 3 * cs + c * cs + z * s_z + ky * s_ky + (kx / LANES) * s_g + kx % LANES,
+// tensor element (c6, kz, ky, kx) at c6 * kcs + kz * k_skz + ky * k_sky + (kx / LANES) * k_sg + kx % LANES
+// (complex / real elements), which covers the row-major and the tiled layouts of fe_api.cu.
 struct Z2Args {
     const void* tw;
     const DevMember* members;
-    int My, pitch, nz, batch;
-    int ngroups;      // pitch / LANES
+    int My, batch;
+    int ngroups;      // groups of LANES consecutive kx
     int nitems;       // ngroups * (My/2 + 1)
+    int64_t cs, s_z, s_ky, s_g;
+    int64_t kcs, k_skz, k_sky, k_sg;
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
@@ -110,14 +115,12 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     cx<T>* stage = buf + 3 * TILE;                                  // staged input [3][NIN][LANES]
     T* kbuf = reinterpret_cast<T*>(stage + 3 * NIN * LANES);        // K~ tile [6][HZ][LANES]
     const int lane = threadIdx.x % LANES, tp = threadIdx.x / LANES;
-    const int64_t sa = (int64_t)a.My * a.pitch, cs = (int64_t)a.nz * sa;
-    const int Hy = a.My / 2 + 1;
-    const int64_t kcs = (int64_t)HZ * Hy * a.pitch;
+    const int64_t sa = a.s_z, cs = a.cs, kcs = a.kcs;
 
     auto tile_base = [&](const ZIter& it) -> cx<T>* {
         int b, ky;
         it.tile(a, b, ky);
-        return S + (int64_t)b * 3 * cs + (int64_t)ky * a.pitch + it.kxg * LANES;
+        return S + (int64_t)b * 3 * cs + (int64_t)ky * a.s_ky + (int64_t)it.kxg * a.s_g;
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
     auto prefetch_tile = [&](const ZIter& it) {
@@ -143,8 +146,8 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         constexpr int RSTEP = C::THREADS / OPS_ROW;
         static_assert(LANES * sizeof(T) >= 8 && C::THREADS % OPS_ROW == 0, "a K~ row of a tile must be at least 8 bytes");
         const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
-        const int64_t krs = (int64_t)Hy * a.pitch;                      // stride of kz in the table
-        const T* g = Kt + (int64_t)it.kyh * a.pitch + it.kxg * LANES + (int64_t)row0 * krs + q * PER;
+        const int64_t krs = a.k_skz;                                    // stride of kz in the table
+        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)it.kxg * a.k_sg + (int64_t)row0 * krs + q * PER;
         T* s = kbuf + row0 * LANES + q * PER;
 #pragma unroll
         for (int c6 = 0; c6 < 6; ++c6) {
@@ -282,7 +285,6 @@ static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
             return e;
         nblocks = sms * (per > 0 ? per : 1);
     }
-    a.ngroups = a.pitch / LANES;
     a.nitems = a.ngroups * (a.My / 2 + 1);
     const int grid = a.nitems < nblocks ? a.nitems : nblocks;
     k2_zmul<T, M, LANES, PRUNE><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a);
@@ -299,14 +301,15 @@ static cudaError_t launch_p(bool prune, void* S, const T* Kt, const Z2Args& a, c
 
 bool zmul2_supported(int M) { return M == 64 || M == 128 || M == 256; }
 
-// same contract as launch_zmul (fe_fft.cu); pitch must be a multiple of 128 bytes of complex elements
+// fused z pass in place on the spectra; strides as in Z2Args (ngroups groups of 128 bytes of consecutive kx)
 template <typename T>
-cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int pitch,
-                         int batch, cudaStream_t st)
+cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
+                         int batch, const int64_t sstr[4], const int64_t kstr[4], cudaStream_t st)
 {
     const int M = c.plan[2].M;
     constexpr int L128 = 128 / (int)sizeof(v2::cx<T>);      // lanes of a 128-byte row
-    v2::Z2Args a{c.tw, members, My, pitch, nz, batch, 0, 0};
+    v2::Z2Args a{c.tw, members, My, batch, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
+                 kstr[0], kstr[1], kstr[2], kstr[3]};
     const bool prune = 2 * nz == M;
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
@@ -316,7 +319,11 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
             // 128-byte rows (one 256-thread block per SM) beat 64-byte rows (two 128-thread blocks) on B200:
             // 0.66 vs 0.80 ms at cfg5a.  FE_B200_ZLANES=4 selects the narrow tile (tuning aid).
             static const int zl = getenv("FE_B200_ZLANES") ? atoi(getenv("FE_B200_ZLANES")) : 0;
-            if (zl == 4 || sizeof(T) != 8) return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
+            if (zl == 4 && a.s_g == L128 && a.k_sg == L128) {
+                // half-width tiles (row-major spectra only): twice the groups, half the group stride
+                a.ngroups *= 2; a.s_g /= 2; a.k_sg /= 2;
+                return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
+            }
             return v2::launch_p<T, 256, L128>(prune, S, Kt, a, st);
         }
         default: return cudaErrorInvalidValue;
@@ -324,8 +331,8 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
 }
 
 template cudaError_t launch_zmul2<double>(const FftCtx&, void*, const double*, const DevMember*, int, int, int, int,
-                                          cudaStream_t);
+                                          const int64_t*, const int64_t*, cudaStream_t);
 template cudaError_t launch_zmul2<float>(const FftCtx&, void*, const float*, const DevMember*, int, int, int, int,
-                                         cudaStream_t);
+                                         const int64_t*, const int64_t*, cudaStream_t);
 
 }  // namespace fe

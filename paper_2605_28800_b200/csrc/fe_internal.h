@@ -87,7 +87,7 @@ cudaError_t launch_zmul(const FftCtx& c, void* S, const T* Kt, const DevMember* 
 // complex fp64 box spectrum -> real octant table of T (scaled)
 template <typename T>
 cudaError_t launch_extract(const void* Sbox, T* Kt_comp, int Mz, int My, int Lx, int pitch64, int pitchT,
-                           double scale, cudaStream_t st);
+                           double scale, int lanes, int64_t k_skz, int64_t k_sky, int64_t k_sg, cudaStream_t st);
 size_t zmul_smem_bytes(int Mz, int lanes, size_t cx_bytes);
 
 // ---- size-specialised register FFT passes (fe_fft2_*.cu); same data layouts as the generic launchers above
@@ -96,17 +96,18 @@ bool axis2_supported(int M);
 bool zmul2_supported(int M);
 template <typename T>
 cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, int64_t nrows, int64_t real_rs,
-                         int64_t spec_rs, cudaStream_t st);
+                         const int64_t spec[4] /* ny, s_plane, s_row, s_g */, int lanes, cudaStream_t st);
 template <typename T>
-cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t spec_rs,
-                         int64_t real_rs, cudaStream_t st);
+cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t real_rs,
+                         const int64_t spec[4], int lanes, cudaStream_t st);
 template <typename T>
-cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int pitch_used,
-                         int outer, int batch, int64_t in_sa, int64_t in_so, int64_t in_sb, int64_t out_sa,
-                         int64_t out_so, int64_t out_sb, cudaStream_t st);
+cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int n0, int n1,
+                         int batch, int64_t in_sa, int64_t in_s0, int64_t in_s1, int64_t in_sb, int64_t out_sa,
+                         int64_t out_s0, int64_t out_s1, int64_t out_sb, cudaStream_t st);
 template <typename T>
-cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int pitch,
-                         int batch, cudaStream_t st);
+cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
+                         int batch, const int64_t sstr[4] /* cs, s_z, s_ky, s_g */,
+                         const int64_t kstr[4] /* kcs, k_skz, k_sky, k_sg */, cudaStream_t st);
 cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
 
 // ---- tensor (fe_tensor.cu) --------------------------------------------------------------------
