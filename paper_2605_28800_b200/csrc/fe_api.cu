@@ -216,7 +216,8 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
         g->fast[2] = !generic && zmul2_supported(q.m[2]) && (size_t)q.lanes == lanes_full;
         // Tiled layouts (L = 128 bytes of consecutive kx, G = pitch / L groups), used when every pass is fast:
         //   S1[b][c][z][g][y][L]   the y pass reads / writes whole contiguous tiles,
-        //   S2[b][c][g][ky][z][L]  the fused z pass works on contiguous tiles (no 2 MB strides),
+        //   S2[b][c][g][z][ky][L]  likewise (ky in slot order when the bulk-copy y pass runs); the fused z pass reads
+        //                          128-byte rows 64 KB apart instead of 2 MB apart,
         //   Kt[6][g][ky][kz][L]    its tensor tile is contiguous too.
         // FE_B200_LINEAR=1 keeps the row-major layouts (tuning aid).
         const char* lin = getenv("FE_B200_LINEAR");
@@ -494,9 +495,15 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     // strides (complex elements; the tensor table in reals), row-major or tiled (see fe_create_grid)
     const int64_t xspec[4] = {ny, p * ny, tl ? L : p, tl ? (int64_t)ny * L : L};             // S1 as the x passes see it
     const int64_t y1_sa = tl ? L : p, y1_sg = tl ? (int64_t)ny * L : L, y1_sz = p * ny, y1_sb = p * ny * nz;   // S1, y pass
-    const int64_t y2_sa = tl ? (int64_t)nz * L : p, y2_sg = tl ? (int64_t)My * nz * L : L, y2_sz = tl ? L : p * My,
+    // tiled S2[b][c][g][z][ky][L]: the y pass reads and writes whole contiguous tiles
+    const int64_t y2_sa = tl ? L : p, y2_sg = tl ? (int64_t)My * nz * L : L, y2_sz = tl ? (int64_t)My * L : p * My,
                   y2_sb = p * My * nz;                                                          // S2, y pass
-    const int64_t zs[4] = {p * My * nz, tl ? L : p * My, tl ? (int64_t)nz * L : p, tl ? (int64_t)My * nz * L : L};
+    const int64_t zs[4] = {p * My * nz, tl ? (int64_t)My * L : p * My, tl ? L : p, tl ? (int64_t)My * nz * L : L};
+    // bulk-copy y pass (contiguous tiles, ky of S2 in slot order); FE_B200_Y4=0 falls back to the register-I/O pass
+    static const bool y4off = getenv("FE_B200_Y4") && getenv("FE_B200_Y4")[0] == '0';
+    const bool use4 = tl && !y4off && axis4_supported(My);
+    int perm[3] = {0, 0, 0};
+    if (use4) axis4_radices(My, perm);
     const int64_t ks[4] = {(int64_t)Hz * Hy * p, tl ? L : (int64_t)Hy * p, tl ? (int64_t)Hz * L : p,
                            tl ? (int64_t)Hy * Hz * L : L};
     mark(g, K_XFWD, st);
@@ -505,7 +512,8 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     mark(g, K_YFWD, st);
     if (g->fast[1]) {
         // tiled: z is the fastest block index, so that concurrently running blocks write neighbouring 128-byte pieces
-        if (tl) FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, ny, nz, G, B * 3, y1_sa, y1_sz, y1_sg, y1_sb,
+        if (use4) FE_CUDA(launch_axis4<T>(g->ctx, 1, -1, S1, S2, ny, nz, G, B * 3, y1_sz, y1_sg, y1_sb, y2_sz, y2_sg, y2_sb, st));
+        else if (tl) FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, ny, nz, G, B * 3, y1_sa, y1_sz, y1_sg, y1_sb,
                                         y2_sa, y2_sz, y2_sg, y2_sb, st));
         else FE_CUDA(launch_axis2<T>(g->ctx, 1, -1, S1, S2, ny, G, nz, B * 3, y1_sa, y1_sg, y1_sz, y1_sb,
                                      y2_sa, y2_sg, y2_sz, y2_sb, st));
@@ -514,11 +522,12 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
                                p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
     }
     mark(g, K_ZMUL, st);
-    if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, st));
+    if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, st));
     else FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
     mark(g, K_YINV, st);
     if (g->fast[1]) {
-        if (tl) FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, ny, nz, G, B * 3, y2_sa, y2_sz, y2_sg, y2_sb,
+        if (use4) FE_CUDA(launch_axis4<T>(g->ctx, 1, +1, S2, S1, ny, nz, G, B * 3, y2_sz, y2_sg, y2_sb, y1_sz, y1_sg, y1_sb, st));
+        else if (tl) FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, ny, nz, G, B * 3, y2_sa, y2_sz, y2_sg, y2_sb,
                                         y1_sa, y1_sz, y1_sg, y1_sb, st));
         else FE_CUDA(launch_axis2<T>(g->ctx, 1, +1, S2, S1, ny, G, nz, B * 3, y2_sa, y2_sg, y2_sz, y2_sb,
                                      y1_sa, y1_sg, y1_sz, y1_sb, st));

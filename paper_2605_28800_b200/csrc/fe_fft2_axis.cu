@@ -185,6 +185,254 @@ static cudaError_t launch_m3(int dir, bool prune, const void* in, void* out, con
     return prune ? launch_one3<T, M, +1, true>(in, out, a, grid, st) : launch_one3<T, M, +1, false>(in, out, a, grid, st);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Bulk-copy variant for contiguous tiles (tiled layouts of fe_api.cu, M = 256 or 512): persistent blocks, a ring
+// of three M x 128-byte buffers per block.  A tile arrives with one cp.async.bulk (mbarrier completion), is
+// transformed IN PLACE by the three-level scheme above (every task writes exactly the slots it read), and leaves
+// with one cp.async.bulk store, so loads of tile i+2, the transform of tile i and the store of tile i-1 overlap
+// and no data passes through registers on its way to or from HBM.
+//   forward: input row y at slot y; output frequency k = k1 + RA k2 + RA RB k3 at slot (k1 RB + k2) RC + k3
+//            ("slot order": the digit-reversed ky order in which S2 is stored when this kernel is used),
+//   inverse: input in slot order, levels run C', B', A'; output row y at slot y.
+// ------------------------------------------------------------------------------------------------
+struct Axis4Args {
+    const void* tw;
+    int n0, n1, ntiles;                   // tile t -> (t % n0, (t / n0) % n1, t / (n0 n1))
+    int64_t in_s0, in_s1, in_sb, out_s0, out_s1, out_sb;
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity)
+{
+    const unsigned addr = smem_u32(bar);
+    unsigned done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, void* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* gdst, const void* smem_src, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n" ::"l"(gdst), "r"(smem_u32(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;\n" ::: "memory");
+}
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;\n" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
+template <typename T, int M, int DIR, bool PRUNE, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1)
+k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
+{
+    constexpr int RA = Fact3<M>::RA, RB = Fact3<M>::RB, RC = Fact3<M>::RC;
+    constexpr int LANES = 128 / (int)sizeof(cx<T>);
+    constexpr int TPP = THREADS / LANES;
+    constexpr int NTA = RB * RC, NTB = RA * RC, NTC = RA * RB;
+    static_assert(NTA % TPP == 0 && NTB % TPP == 0 && NTC % TPP == 0, "tasks must divide evenly");
+    constexpr int NB = 3;
+    constexpr int TILE = M * LANES;
+    constexpr bool PIN = PRUNE && DIR < 0, POUT = PRUNE && DIR > 0;
+    constexpr unsigned in_bytes = (unsigned)((PIN ? M / 2 : M) * LANES * sizeof(cx<T>));
+    constexpr unsigned out_bytes = (unsigned)((POUT ? M / 2 : M) * LANES * sizeof(cx<T>));
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(fe2_smem);     // [NB], 64 bytes reserved
+    cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem + 64);
+    cx<T>* bufs = tw + M;
+    const int lane = threadIdx.x % LANES, tp = threadIdx.x / LANES;
+
+    auto in_ptr = [&](int t) {
+        const int i0 = t % a.n0, r = t / a.n0, i1 = r % a.n1, ib = r / a.n1;
+        return in + (int64_t)ib * a.in_sb + (int64_t)i1 * a.in_s1 + (int64_t)i0 * a.in_s0;
+    };
+    auto out_ptr = [&](int t) {
+        const int i0 = t % a.n0, r = t / a.n0, i1 = r % a.n1, ib = r / a.n1;
+        return out + (int64_t)ib * a.out_sb + (int64_t)i1 * a.out_s1 + (int64_t)i0 * a.out_s0;
+    };
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NB; ++b) mbar_init(&bars[b], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, THREADS);
+    __syncthreads();
+    const int t0 = blockIdx.x, dt = gridDim.x;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int pre = 0; pre < 2; ++pre) {
+            const int t = t0 + pre * dt;
+            if (t < a.ntiles) {
+                mbar_expect_tx(&bars[pre], in_bytes);
+                bulk_load(bufs + pre * TILE, in_ptr(t), in_bytes, &bars[pre]);
+            }
+        }
+    }
+    int i = 0;
+    for (int t = t0; t < a.ntiles; t += dt, ++i) {
+        const int b = i % NB;
+        cx<T>* buf = bufs + b * TILE + lane;
+        mbar_wait(&bars[b], (unsigned)((i / NB) & 1));
+        if (DIR < 0) {
+            // ---- A: task j = n3 + RC n2, slots j + RB RC n1
+#pragma unroll
+            for (int it = 0; it < NTA / TPP; ++it) {
+                const int j = tp + it * TPP;
+                cx<T> u[RA];
+                cx<T>* col = buf + j * LANES;
+                static_for<(PIN ? RA / 2 : RA)>([&](auto ic) { u[decltype(ic)::value] = col[decltype(ic)::value * RB * RC * LANES]; });
+                Dif<T, DIR, RA, 0, PIN>::run(u);
+                static_for<RA>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int k1 = brev<RA>(p);
+                    cx<T> val = u[p];
+                    if constexpr (k1 != 0) val = cmul(val, tw[j * k1]);
+                    col[k1 * RB * RC * LANES] = val;
+                });
+            }
+            __syncthreads();
+            // ---- B: task (k1, n3), slots k1 RB RC + n3 + RC n2
+#pragma unroll
+            for (int it = 0; it < NTB / TPP; ++it) {
+                const int tb = tp + it * TPP, n3 = tb % RC, k1 = tb / RC;
+                cx<T> u[RB];
+                cx<T>* col = buf + (k1 * RB * RC + n3) * LANES;
+                static_for<RB>([&](auto nc) { u[decltype(nc)::value] = col[decltype(nc)::value * RC * LANES]; });
+                Dif<T, DIR, RB>::run(u);
+                static_for<RB>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int k2 = brev<RB>(p);
+                    cx<T> val = u[p];
+                    if constexpr (k2 != 0) val = cmul(val, tw[RA * n3 * k2]);
+                    col[k2 * RC * LANES] = val;
+                });
+            }
+            __syncthreads();
+            // ---- C: task tc = k1 RB + k2, slots tc RC + n3
+#pragma unroll
+            for (int it = 0; it < NTC / TPP; ++it) {
+                const int tc = tp + it * TPP;
+                cx<T> u[RC];
+                cx<T>* col = buf + tc * RC * LANES;
+                static_for<RC>([&](auto nc) { u[decltype(nc)::value] = col[decltype(nc)::value * LANES]; });
+                Dif<T, DIR, RC>::run(u);
+                static_for<RC>([&](auto pc) { col[brev<RC>(decltype(pc)::value) * LANES] = u[decltype(pc)::value]; });
+            }
+        } else {
+            // ---- C': task tc = k1 RB + k2 (k2 = tc % RB), slots tc RC + k3 -> n3
+#pragma unroll
+            for (int it = 0; it < NTC / TPP; ++it) {
+                const int tc = tp + it * TPP, k2 = tc % RB;
+                cx<T> u[RC];
+                cx<T>* col = buf + tc * RC * LANES;
+                static_for<RC>([&](auto nc) { u[decltype(nc)::value] = col[decltype(nc)::value * LANES]; });
+                Dif<T, DIR, RC>::run(u);
+                static_for<RC>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int n3 = brev<RC>(p);
+                    cx<T> val = u[p];
+                    if constexpr (n3 != 0) val = cmulc(val, tw[RA * n3 * k2]);
+                    col[n3 * LANES] = val;
+                });
+            }
+            __syncthreads();
+            // ---- B': task (k1, n3), slots k1 RB RC + n3 + RC k2 -> n2
+#pragma unroll
+            for (int it = 0; it < NTB / TPP; ++it) {
+                const int tb = tp + it * TPP, n3 = tb % RC, k1 = tb / RC;
+                cx<T> u[RB];
+                cx<T>* col = buf + (k1 * RB * RC + n3) * LANES;
+                static_for<RB>([&](auto nc) { u[decltype(nc)::value] = col[decltype(nc)::value * RC * LANES]; });
+                Dif<T, DIR, RB>::run(u);
+                static_for<RB>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int n2 = brev<RB>(p);
+                    col[n2 * RC * LANES] = cmulc(u[p], tw[(n3 + RC * n2) * k1]);
+                });
+            }
+            __syncthreads();
+            // ---- A': task j = n3 + RC n2, slots j + RB RC k1 -> n1 (first half kept when pruned)
+#pragma unroll
+            for (int it = 0; it < NTA / TPP; ++it) {
+                const int j = tp + it * TPP;
+                cx<T> u[RA];
+                cx<T>* col = buf + j * LANES;
+                static_for<RA>([&](auto kc) { u[decltype(kc)::value] = col[decltype(kc)::value * RB * RC * LANES]; });
+                Dif<T, DIR, RA>::run(u);
+                static_for<RA>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int n1 = brev<RA>(p);
+                    if constexpr (!POUT || n1 < RA / 2) col[n1 * RB * RC * LANES] = u[p];
+                });
+            }
+        }
+        fence_async_smem();                 // generic-proxy writes of this thread -> visible to the bulk store
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            bulk_store(out_ptr(t), bufs + b * TILE, out_bytes);
+            // the buffer of tile i-1 is reused for tile i+2: its store must have finished reading shared memory
+            const int tn = t + 2 * dt;
+            if (tn < a.ntiles) {
+                bulk_wait_read<1>();
+                const int bn = (i + 2) % NB;
+                mbar_expect_tx(&bars[bn], in_bytes);
+                bulk_load(bufs + bn * TILE, in_ptr(tn), in_bytes, &bars[bn]);
+            }
+        }
+    }
+    if (threadIdx.x == 0) bulk_wait_read<0>();
+}
+
+template <typename T, int M, int DIR, bool PRUNE, int THREADS>
+static cudaError_t launch_one4(const void* in, void* out, Axis4Args a, cudaStream_t st)
+{
+    constexpr int LANES = 128 / (int)sizeof(cx<T>);
+    constexpr size_t smem = 64 + (size_t)(M + 3 * M * LANES) * sizeof(cx<T>);
+    static int nblocks = 0;
+    if (!nblocks) {
+        cudaError_t e = cudaFuncSetAttribute(k4_axis<T, M, DIR, PRUNE, THREADS>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        int dev = 0, sms = 0, per = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k4_axis<T, M, DIR, PRUNE, THREADS>, THREADS, smem)) !=
+            cudaSuccess)
+            return e;
+        nblocks = sms * (per > 0 ? per : 1);
+    }
+    const int grid = a.ntiles < nblocks ? a.ntiles : nblocks;
+    k4_axis<T, M, DIR, PRUNE, THREADS><<<grid, THREADS, smem, st>>>(static_cast<const cx<T>*>(in), static_cast<cx<T>*>(out), a);
+    return cudaGetLastError();
+}
+
+template <typename T, int M, int THREADS>
+static cudaError_t launch_m4(int dir, bool prune, const void* in, void* out, const Axis4Args& a, cudaStream_t st)
+{
+    if (dir < 0) return prune ? launch_one4<T, M, -1, true, THREADS>(in, out, a, st)
+                              : launch_one4<T, M, -1, false, THREADS>(in, out, a, st);
+    return prune ? launch_one4<T, M, +1, true, THREADS>(in, out, a, st) : launch_one4<T, M, +1, false, THREADS>(in, out, a, st);
+}
+
 template <typename T, int M, int DIR, bool PRUNE>
 static cudaError_t launch_one(const void* in, void* out, const Axis2Args& a, dim3 grid, cudaStream_t st)
 {
@@ -240,6 +488,46 @@ cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, voi
         default: return cudaErrorInvalidValue;
     }
 }
+
+bool axis4_supported(int M) { return M == 256 || M == 512; }
+
+// slot of frequency k in the output of the bulk-copy pass (and of its input in the inverse direction)
+int axis4_slot(int M, int k)
+{
+    int RA, RB, RC;
+    if (M == 512) { RA = v2::Fact3<512>::RA; RB = v2::Fact3<512>::RB; RC = v2::Fact3<512>::RC; }
+    else { RA = v2::Fact3<256>::RA; RB = v2::Fact3<256>::RB; RC = v2::Fact3<256>::RC; }
+    const int k1 = k % RA, k2 = (k / RA) % RB, k3 = k / (RA * RB);
+    return (k1 * RB + k2) * RC + k3;
+}
+void axis4_radices(int M, int r[3])
+{
+    if (M == 512) { r[0] = v2::Fact3<512>::RA; r[1] = v2::Fact3<512>::RB; r[2] = v2::Fact3<512>::RC; }
+    else { r[0] = v2::Fact3<256>::RA; r[1] = v2::Fact3<256>::RB; r[2] = v2::Fact3<256>::RC; }
+}
+
+// Bulk-copy pass over contiguous tiles: tile (i0, i1, ib) of the input starts at i0 in_s0 + i1 in_s1 + ib in_sb and
+// holds n_keep (forward) or M (inverse) rows of 128 bytes back to back; the output tile likewise.  The spectrum
+// side is in slot order (axis4_slot).
+template <typename T>
+cudaError_t launch_axis4(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int n0, int n1,
+                         int batch, int64_t in_s0, int64_t in_s1, int64_t in_sb, int64_t out_s0, int64_t out_s1,
+                         int64_t out_sb, cudaStream_t st)
+{
+    const int M = c.plan[axis].M;
+    const bool prune = 2 * n_keep == M;
+    if (!prune && n_keep != M) return cudaErrorInvalidValue;
+    v2::Axis4Args a{c.tw, n0, n1, n0 * n1 * batch, in_s0, in_s1, in_sb, out_s0, out_s1, out_sb};
+    static const bool t512 = getenv("FE_B200_Y4T") && atoi(getenv("FE_B200_Y4T")) == 512;   // tuning aid
+    if (M == 256) return v2::launch_m4<T, 256, 256>(dir, prune, in, out, a, st);
+    if (M == 512) return t512 ? v2::launch_m4<T, 512, 512>(dir, prune, in, out, a, st) : v2::launch_m4<T, 512, 256>(dir, prune, in, out, a, st);
+    return cudaErrorInvalidValue;
+}
+
+template cudaError_t launch_axis4<double>(const FftCtx&, int, int, const void*, void*, int, int, int, int, int64_t,
+                                          int64_t, int64_t, int64_t, int64_t, int64_t, cudaStream_t);
+template cudaError_t launch_axis4<float>(const FftCtx&, int, int, const void*, void*, int, int, int, int, int64_t,
+                                         int64_t, int64_t, int64_t, int64_t, int64_t, cudaStream_t);
 
 template cudaError_t launch_axis2<double>(const FftCtx&, int, int, const void*, void*, int, int, int, int, int64_t,
                                           int64_t, int64_t, int64_t, int64_t, int64_t, int64_t, int64_t, cudaStream_t);

@@ -35,6 +35,7 @@ struct Z2Args {
     int nitems;       // ngroups * (My/2 + 1)
     int64_t cs, s_z, s_ky, s_g;
     int64_t kcs, k_skz, k_sky, k_sg;
+    int pa, pb, pc;   // ky is stored in slot order (k1 pb + k2) pc + k3, ky = k1 + pa k2 + pa pb k3; pa = 0: natural
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
@@ -120,7 +121,9 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     auto tile_base = [&](const ZIter& it) -> cx<T>* {
         int b, ky;
         it.tile(a, b, ky);
-        return S + (int64_t)b * 3 * cs + (int64_t)ky * a.s_ky + (int64_t)it.kxg * a.s_g;
+        int slot = ky;
+        if (a.pa) slot = ((ky % a.pa) * a.pb + (ky / a.pa) % a.pb) * a.pc + ky / (a.pa * a.pb);
+        return S + (int64_t)b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)it.kxg * a.s_g;
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
     auto prefetch_tile = [&](const ZIter& it) {
@@ -304,12 +307,12 @@ bool zmul2_supported(int M) { return M == 64 || M == 128 || M == 256; }
 // fused z pass in place on the spectra; strides as in Z2Args (ngroups groups of 128 bytes of consecutive kx)
 template <typename T>
 cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
-                         int batch, const int64_t sstr[4], const int64_t kstr[4], cudaStream_t st)
+                         int batch, const int64_t sstr[4], const int64_t kstr[4], const int perm[3], cudaStream_t st)
 {
     const int M = c.plan[2].M;
     constexpr int L128 = 128 / (int)sizeof(v2::cx<T>);      // lanes of a 128-byte row
     v2::Z2Args a{c.tw, members, My, batch, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
-                 kstr[0], kstr[1], kstr[2], kstr[3]};
+                 kstr[0], kstr[1], kstr[2], kstr[3], perm[0], perm[1], perm[2]};
     const bool prune = 2 * nz == M;
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
@@ -331,8 +334,8 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
 }
 
 template cudaError_t launch_zmul2<double>(const FftCtx&, void*, const double*, const DevMember*, int, int, int, int,
-                                          const int64_t*, const int64_t*, cudaStream_t);
+                                          const int64_t*, const int64_t*, const int*, cudaStream_t);
 template cudaError_t launch_zmul2<float>(const FftCtx&, void*, const float*, const DevMember*, int, int, int, int,
-                                         const int64_t*, const int64_t*, cudaStream_t);
+                                         const int64_t*, const int64_t*, const int*, cudaStream_t);
 
 }  // namespace fe

@@ -104,10 +104,18 @@ template <typename T>
 cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int n0, int n1,
                          int batch, int64_t in_sa, int64_t in_s0, int64_t in_s1, int64_t in_sb, int64_t out_sa,
                          int64_t out_s0, int64_t out_s1, int64_t out_sb, cudaStream_t st);
+bool axis4_supported(int M);
+int axis4_slot(int M, int k);
+void axis4_radices(int M, int r[3]);
+template <typename T>
+cudaError_t launch_axis4(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int n0, int n1,
+                         int batch, int64_t in_s0, int64_t in_s1, int64_t in_sb, int64_t out_s0, int64_t out_s1,
+                         int64_t out_sb, cudaStream_t st);
 template <typename T>
 cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
                          int batch, const int64_t sstr[4] /* cs, s_z, s_ky, s_g */,
-                         const int64_t kstr[4] /* kcs, k_skz, k_sky, k_sg */, cudaStream_t st);
+                         const int64_t kstr[4] /* kcs, k_skz, k_sky, k_sg */,
+                         const int perm[3] /* slot-order radices of ky, {0,0,0}: natural */, cudaStream_t st);
 cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
 
 // ---- tensor (fe_tensor.cu) --------------------------------------------------------------------
