@@ -302,6 +302,286 @@ __global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// k_local2: the same z-marching scheme with a 64 x 8 column per block and TWO x-adjacent cells per thread.
+// Interior cell x of the tile sits at column 2 + x of a 68-wide shared row, so the pair (2 tx, 2 tx + 1) is a
+// 16-byte (fp64) aligned vector: centre, y and z taps of both cells come with one vector load each, which
+// halves the shared-memory instructions per cell; the plane loader moves pairs as well.
+// ------------------------------------------------------------------------------------------------
+constexpr int k2TX = 64, k2PX = 68, k2HY = kTY + 2, k2Tile = k2PX * k2HY;        // 68 x 10 = 680
+constexpr int k2Pairs = k2HY * (k2TX / 2);                                      // pair entries per component
+constexpr int k2Sing = k2HY * 2;                                                // halo-column entries per component
+constexpr int k2NL = (3 * (k2Pairs + k2Sing) + 255) / 256;                      // loader entries per thread (4)
+
+template <typename T> struct alignas(2 * sizeof(T)) pair_t { T a, b; };
+
+template <typename T, bool MAP, bool MIXED>
+__global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
+{
+    extern __shared__ __align__(16) unsigned char lsm[];
+    T* tiles = reinterpret_cast<T*>(lsm);                                   // [4][3][k2Tile]
+    unsigned char* flags = lsm + (size_t)4 * 3 * k2Tile * sizeof(T);        // [4][k2Tile]
+    LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + 4 * k2Tile);   // [nmat]
+    unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
+    using P2 = pair_t<T>;
+
+    const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
+    const int ntx = (nx + k2TX - 1) / k2TX;
+    const int x0 = (blockIdx.x % ntx) * k2TX, y0 = (blockIdx.x / ntx) * kTY;
+    const int z0 = blockIdx.y * a.zchunk, z1 = min(z0 + a.zchunk, nz);
+    const int b = blockIdx.z;
+    const int t = threadIdx.x, tx = t & 31, ty = t >> 5;
+    const int64_t nxy = (int64_t)nx * ny, N = nxy * nz;
+    const T* Y = static_cast<const T*>(a.Y) + (int64_t)b * 3 * N;
+    const DevLandau* mats = a.mats + (int64_t)b * a.nmat;
+    for (int m = t; m < a.nmat; m += 256) {
+        smats[m] = LandauD<T>(mats[m]);
+        sact[m] = mats[m].active != 0;
+    }
+    const DevMember mem = a.members[b];
+
+    // loader entries: shared offset (-1: none), in-plane global offset of the first cell (-1: outside), pair or single
+    int l_so[k2NL], l_go[k2NL];
+    bool l_pair[k2NL];
+    const T* l_ptr[k2NL];
+#pragma unroll
+    for (int k = 0; k < k2NL; ++k) {
+        const int idx = t + 256 * k;
+        l_so[k] = -1;
+        l_go[k] = -1;
+        l_pair[k] = false;
+        l_ptr[k] = Y;
+        int comp = 0, yy = 0, col = 0;
+        bool have = false;
+        if (idx < 3 * k2Pairs) {
+            comp = idx / k2Pairs;
+            const int rem = idx % k2Pairs;
+            yy = rem / (k2TX / 2);
+            col = 2 * (rem % (k2TX / 2));            // tile x of the first cell of the pair
+            l_pair[k] = true;
+            have = true;
+        } else if (idx < 3 * (k2Pairs + k2Sing)) {
+            const int s2 = idx - 3 * k2Pairs;
+            comp = s2 / k2Sing;
+            const int rem = s2 % k2Sing;
+            yy = rem / 2;
+            col = (rem & 1) ? k2TX : -1;
+            have = true;
+        }
+        if (have) {
+            int gx = x0 + col, gy = y0 - 1 + yy;
+            bool in = true;
+            if (gx < 0 || gx >= nx) { if (a.periodic[0]) gx = ((gx % nx) + nx) % nx; else in = false; }
+            if (gy < 0 || gy >= ny) { if (a.periodic[1]) gy = ((gy % ny) + ny) % ny; else in = false; }
+            l_so[k] = comp * k2Tile + yy * k2PX + 2 + col;
+            l_go[k] = in ? gy * nx + gx : -1;
+            if (in) l_ptr[k] = Y + (int64_t)comp * N + l_go[k];
+        }
+    }
+    T pre[k2NL][2];
+    bool pok[k2NL][2];
+    auto fetch_plane = [&](int z) {
+        int zz = z;
+        bool zin = true;
+        if (zz < 0 || zz >= nz) { if (a.periodic[2]) zz = ((zz % nz) + nz) % nz; else zin = false; }
+        const int64_t r0 = (int64_t)zz * nxy;
+#pragma unroll
+        for (int k = 0; k < k2NL; ++k) {
+            const bool ok = zin && l_go[k] >= 0;
+            pre[k][0] = pre[k][1] = (T)0;
+            pok[k][0] = pok[k][1] = ok;
+            if (ok) {
+                if (l_pair[k]) {
+                    const P2 v = *reinterpret_cast<const P2*>(l_ptr[k] + r0);
+                    pre[k][0] = v.a;
+                    pre[k][1] = v.b;
+                } else {
+                    pre[k][0] = l_ptr[k][r0];
+                }
+                if (MAP) {
+                    pok[k][0] = sact[a.map[r0 + l_go[k]]] != 0;
+                    if (l_pair[k]) pok[k][1] = sact[a.map[r0 + l_go[k] + 1]] != 0;
+                }
+            }
+        }
+    };
+    auto store_plane = [&](int z) {
+        const int slot = z & 3;
+        T* tl = tiles + slot * 3 * k2Tile;
+        unsigned char* fl = flags + slot * k2Tile;
+#pragma unroll
+        for (int k = 0; k < k2NL; ++k) {
+            if (l_so[k] < 0) continue;
+            if (l_pair[k]) {
+                *reinterpret_cast<P2*>(tl + l_so[k]) = P2{pok[k][0] ? pre[k][0] : (T)0, pok[k][1] ? pre[k][1] : (T)0};
+                if (MAP && l_so[k] < k2Tile) { fl[l_so[k]] = pok[k][0]; fl[l_so[k] + 1] = pok[k][1]; }
+            } else {
+                tl[l_so[k]] = pok[k][0] ? pre[k][0] : (T)0;
+                if (MAP && l_so[k] < k2Tile) fl[l_so[k]] = pok[k][0];
+            }
+        }
+    };
+    __syncthreads();          // coefficient tables visible (fetch_plane reads sact)
+    fetch_plane(z0 - 1);
+    store_plane(z0 - 1);
+    fetch_plane(z0);
+    store_plane(z0);
+    fetch_plane(z0 + 1);
+
+    const int x = x0 + 2 * tx, y = y0 + ty;          // cells (x, y) and (x + 1, y)
+    const bool inside = x < nx && y < ny;            // nx is even: both cells or none
+    const int64_t rxy = (int64_t)y * nx + x;
+    const int c0 = (ty + 1) * k2PX + 2 + 2 * tx;
+    const T gxfA = (T)((x > 0 || a.periodic[0]) + 1), gxfB = (T)(1 + (x + 2 < nx || a.periodic[0]));
+    const T gyf = (T)((y > 0 || a.periodic[1]) + (y < ny - 1 || a.periodic[1]));
+    const T G11 = (T)mem.G11, Gt = (T)mem.Gt, Gm = (T)mem.Gm, L = (T)mem.L;
+    const T ix = (T)a.id2[0], iy = (T)a.id2[1], iz = (T)a.id2[2];
+    const T qxy = Gm * (T)a.i4[0], qxz = Gm * (T)a.i4[1], qyz = Gm * (T)a.i4[2];
+    const T cy = (T)a.cy, ca = (T)a.ca;
+    const T ex0 = (T)mem.Eext[0], ex1 = (T)mem.Eext[1], ex2 = (T)mem.Eext[2];
+    const T* Ee = (a.terms & 4u) && a.Eelec ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
+    const T* base = a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
+    const bool base_is_Y = a.baseY == a.Y;
+    T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
+    const T* ai = a.accOut ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
+    T* ao = a.accOut ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
+    const LandauD<T> lc0 = smats[0];
+    auto ldp = [](const T* q) { return *reinterpret_cast<const P2*>(q); };
+
+    P2 en[3] = {{0, 0}, {0, 0}, {0, 0}};
+    if (Ee && inside) {
+        const int64_t r = (int64_t)z0 * nxy + rxy;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + r);
+    }
+    for (int z = z0; z < z1; ++z) {
+        store_plane(z + 1);
+        __syncthreads();
+        if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
+        if (!inside) continue;
+        const P2 ec[3] = {en[0], en[1], en[2]};
+        if (Ee && z + 1 < z1) {
+            const int64_t rn = (int64_t)(z + 1) * nxy + rxy;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + rn);
+        }
+        const T* m0 = tiles + ((z - 1) & 3) * 3 * k2Tile;     // plane z-1
+        const T* c = tiles + (z & 3) * 3 * k2Tile;            // plane z
+        const T* p1 = tiles + ((z + 1) & 3) * 3 * k2Tile;     // plane z+1
+        const unsigned char* fm = flags + ((z - 1) & 3) * k2Tile;
+        const unsigned char* fc = flags + (z & 3) * k2Tile;
+        const unsigned char* fp = flags + ((z + 1) & 3) * k2Tile;
+        const int64_t r = (int64_t)z * nxy + rxy;
+        const bool actA = !MAP || fc[c0], actB = !MAP || fc[c0 + 1];
+        T EA[3] = {0, 0, 0}, EB[3] = {0, 0, 0};
+        P2 pc[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) pc[i] = ldp(c + i * k2Tile + c0);
+        if (a.terms & 1u) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const LandauD<T> lc = MAP ? smats[a.map[r + h]] : lc0;
+                const T px = h ? pc[0].b : pc[0].a, py = h ? pc[1].b : pc[1].a, pz = h ? pc[2].b : pc[2].a;
+                const T A = px * px, B = py * py, C = pz * pz;
+                const T A2 = A * A, B2 = B * B, C2 = C * C;
+                T A3 = 0, B3 = 0, C3 = 0;
+                if (lc.o8) { A3 = A2 * A; B3 = B2 * B; C3 = C2 * C; }
+                T* E = h ? EB : EA;
+                E[0] -= px * lc.dfd(lc.k1x, A, A2, B + C, B2 + C2, B * C, B3 + C3);
+                E[1] -= py * lc.dfd(lc.k1y, B, B2, C + A, C2 + A2, C * A, C3 + A3);
+                E[2] -= pz * lc.dfd(lc.k1z, C, C2, A + B, A2 + B2, A * B, A3 + B3);
+            }
+        }
+        if (a.terms & 2u) {
+            // number of existing neighbours per axis (a missing neighbour holds 0 in the tile)
+            const T nzg = (T)((z > 0 || a.periodic[2]) + (z < nz - 1 || a.periodic[2]));
+            const T nxA = MAP ? (T)(fc[c0 - 1] + fc[c0 + 1]) : gxfA, nxB = MAP ? (T)(fc[c0] + fc[c0 + 2]) : gxfB;
+            const T nyA = MAP ? (T)(fc[c0 - k2PX] + fc[c0 + k2PX]) : gyf;
+            const T nyB = MAP ? (T)(fc[c0 + 1 - k2PX] + fc[c0 + 1 + k2PX]) : gyf;
+            const T nzA = MAP ? (T)(fm[c0] + fp[c0]) : nzg, nzB = MAP ? (T)(fm[c0 + 1] + fp[c0 + 1]) : nzg;
+            // taps shared by the bond sums and the mixed term: rows y-1 / y+1 of plane z, planes z-1 / z+1 at row y
+            P2 dn[3], up[3], zm[3], zp[3];
+            T lf[3], rt[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const T* ci = c + i * k2Tile + c0;
+                dn[i] = ldp(ci - k2PX);
+                up[i] = ldp(ci + k2PX);
+                zm[i] = ldp(m0 + i * k2Tile + c0);
+                zp[i] = ldp(p1 + i * k2Tile + c0);
+                lf[i] = ci[-1];
+                rt[i] = ci[2];
+                const T gx_ = (i == 0 ? G11 : Gt) * ix, gy_ = (i == 1 ? G11 : Gt) * iy, gz_ = (i == 2 ? G11 : Gt) * iz;
+                EA[i] += gx_ * (lf[i] + pc[i].b - nxA * pc[i].a) + gy_ * (dn[i].a + up[i].a - nyA * pc[i].a) +
+                         gz_ * (zm[i].a + zp[i].a - nzA * pc[i].a);
+                EB[i] += gx_ * (pc[i].a + rt[i] - nxB * pc[i].b) + gy_ * (dn[i].b + up[i].b - nyB * pc[i].b) +
+                         gz_ * (zm[i].b + zp[i].b - nzB * pc[i].b);
+            }
+            if (MIXED) {
+                // Gm sum_{j != i} [P_j(+i+j) - P_j(+i-j) - P_j(-i+j) + P_j(-i-j)] / (4 D_i D_j); columns -1 .. +2 around cell A
+                const T* cxp = c + c0;
+                const T* cyp = c + k2Tile + c0;
+                const T* czm = m0 + 2 * k2Tile + c0;
+                const T* czp = p1 + 2 * k2Tile + c0;
+                // xy: Py and Px on rows y+-1
+                const T yul = cyp[k2PX - 1], yur = cyp[k2PX + 2], ydl = cyp[-k2PX - 1], ydr = cyp[-k2PX + 2];
+                const T xul = cxp[k2PX - 1], xur = cxp[k2PX + 2], xdl = cxp[-k2PX - 1], xdr = cxp[-k2PX + 2];
+                EA[0] += qxy * (up[1].b - dn[1].b - yul + ydl);
+                EB[0] += qxy * (yur - ydr - up[1].a + dn[1].a);
+                EA[1] += qxy * (up[0].b - dn[0].b - xul + xdl);
+                EB[1] += qxy * (xur - xdr - up[0].a + dn[0].a);
+                // xz: Pz and Px on planes z+-1 at row y
+                const T zpl = czp[-1], zpr = czp[2], zml = czm[-1], zmr = czm[2];
+                const T* cxm = m0 + c0;
+                const T* cxq = p1 + c0;
+                const T xpl = cxq[-1], xpr = cxq[2], xml = cxm[-1], xmr = cxm[2];
+                EA[0] += qxz * (zp[2].b - zm[2].b - zpl + zml);
+                EB[0] += qxz * (zpr - zmr - zp[2].a + zm[2].a);
+                EA[2] += qxz * (zp[0].b - zm[0].b - xpl + xml);
+                EB[2] += qxz * (xpr - xmr - zp[0].a + zm[0].a);
+                // yz: Pz and Py on planes z+-1 at rows y+-1
+                const P2 zpu = ldp(czp + k2PX), zpd = ldp(czp - k2PX), zmu = ldp(czm + k2PX), zmd = ldp(czm - k2PX);
+                const T* cym = m0 + k2Tile + c0;
+                const T* cyq = p1 + k2Tile + c0;
+                const P2 ypu = ldp(cyq + k2PX), ypd = ldp(cyq - k2PX), ymu = ldp(cym + k2PX), ymd = ldp(cym - k2PX);
+                EA[1] += qyz * (zpu.a - zmu.a - zpd.a + zmd.a);
+                EB[1] += qyz * (zpu.b - zmu.b - zpd.b + zmd.b);
+                EA[2] += qyz * (ypu.a - ypd.a - ymu.a + ymd.a);
+                EB[2] += qyz * (ypu.b - ypd.b - ymu.b + ymd.b);
+            }
+        }
+        T kA[3] = {0, 0, 0}, kB[3] = {0, 0, 0};
+        if (Ee) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { EA[i] += ec[i].a; EB[i] += ec[i].b; }
+        }
+        if (a.terms & 8u) {
+            EA[0] += ex0; EA[1] += ex1; EA[2] += ex2;
+            EB[0] += ex0; EB[1] += ex1; EB[2] += ex2;
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            if (actA) kA[i] = L * EA[i];
+            if (actB) kB[i] = L * EB[i];
+        }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            P2 bv = {0, 0};
+            if (base) {
+                // Euler: the stage base is the state itself, already in the tile (vacuum cells hold their raw value in memory)
+                if (base_is_Y && actA && actB) bv = pc[i];
+                else bv = ldp(base + i * N + r);
+            }
+            *reinterpret_cast<P2*>(Yout + i * N + r) = P2{bv.a + cy * kA[i], bv.b + cy * kB[i]};
+            if (ao) {
+                const P2 av = ldp(ai + i * N + r);
+                *reinterpret_cast<P2*>(ao + i * N + r) = P2{av.a + ca * kA[i], av.b + ca * kB[i]};
+            }
+        }
+    }
+
+}
+
 template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t st)
 {
     LocalArgs a = a0;
@@ -309,13 +589,15 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     a.i4[0] = 0.25 / (a.d[0] * a.d[1]);
     a.i4[1] = 0.25 / (a.d[0] * a.d[2]);
     a.i4[2] = 0.25 / (a.d[1] * a.d[2]);
-    const int ntx = (a.n[0] + kTX - 1) / kTX, nty = (a.n[1] + kTY - 1) / kTY;
+    const bool two = a.n[0] >= k2TX;      // two cells per thread on rows of at least 64 cells
+    const int ntx = two ? (a.n[0] + k2TX - 1) / k2TX : (a.n[0] + kTX - 1) / kTX, nty = (a.n[1] + kTY - 1) / kTY;
     // z chunk: as long as possible (halo planes are re-read per chunk) while the grid still fills the machine
     int zc = a.n[2];
     while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
     a.zchunk = zc;
     dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
-    const size_t smem = (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
+    const size_t smem = two ? (size_t)4 * 3 * k2Tile * sizeof(T) + 4 * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1)
+                            : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
     static bool configured = false;
     if (!configured) {
         const int lim = 96 * 1024;      // 255 materials need 61 KB
@@ -323,8 +605,23 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local<T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
+        const int lim2 = 128 * 1024;
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e != cudaSuccess) return e;
         configured = true;
+    }
+    if (two) {
+        if (a.map) {
+            if (a.mixed) k_local2<T, true, true><<<grid, 256, smem, st>>>(a);
+            else k_local2<T, true, false><<<grid, 256, smem, st>>>(a);
+        } else {
+            if (a.mixed) k_local2<T, false, true><<<grid, 256, smem, st>>>(a);
+            else k_local2<T, false, false><<<grid, 256, smem, st>>>(a);
+        }
+        return cudaGetLastError();
     }
     if (a.map) {
         if (a.mixed) k_local<T, true, true><<<grid, 256, smem, st>>>(a);

@@ -7,7 +7,7 @@ import pytest
 
 import fe_inputs as fi
 from oracle import fe_oracle as orc
-from gpu_util import rel_l2, oracle_problem
+from gpu_util import rel_l2, oracle_problem, workload_from_random
 
 pytestmark = pytest.mark.gpu
 
@@ -59,6 +59,34 @@ def test_fast_passes_against_oracle_fft(fe, n, periodic, images):
     Ed = orc.field_direct(o.p, o.table(), w.P0[0], targets=t)
     got_e = g.rhs(P, fi.TERM_ELEC).cpu().numpy()[0].reshape(3, -1)[:, t] / w.globals_[0].L
     assert np.max(np.abs(got_e - Ed)) < 1e-10 * np.max(np.abs(Ed))
+    g.close()
+
+
+@pytest.mark.parametrize("n,periodic,images", [
+    ((64, 8, 8), (0, 0, 0), (0, 0, 0)),
+    ((64, 8, 4), (1, 1, 0), (1, 1, 0)),
+    ((128, 4, 8), (0, 1, 1), (0, 2, 2)),
+])
+def test_two_cell_local_kernel_heterogeneous(fe, n, periodic, images):
+    """Rows of >= 64 cells take the two-cells-per-thread local kernel: material map with vacuum cells, Gm != 0,
+    8th-order slots, E_ext, anisotropic cells, batch of 2, every term alone and all together; Heun and RK4 stages."""
+    w = workload_from_random(61, n, periodic, images, batch=2)
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    for b in range(2):
+        o = orc.Oracle(oracle_problem(w, b), elec="direct")
+        for terms in (fi.TERM_LANDAU, fi.TERM_GRADIENT, fi.TERM_ELEC, fi.TERM_EXT, fi.TERM_ALL):
+            got = g.rhs(P, terms).cpu().numpy()[b]
+            want = o.rhs(w.P0[b], terms)
+            assert rel_l2(got, want) < TOL_RHS64, (b, terms)
+            assert np.all(got[:, o.p.active == 0] == 0.0)
+    o = orc.Oracle(oracle_problem(w, 1), elec="direct")
+    for integ in (fi.EULER, fi.HEUN, fi.RK4):
+        Pd = g.state(w.P0)
+        g.step(Pd, 1e-2, 3, integ, fi.TERM_ALL)
+        want = o.step(w.P0[1], 1e-2, 3, integ, fi.TERM_ALL)
+        assert rel_l2(Pd.cpu().numpy()[1], want) < 1e-12, integ
     g.close()
 
 
