@@ -315,13 +315,23 @@ constexpr int k2NL = (3 * (k2Pairs + k2Sing) + 255) / 256;                      
 
 template <typename T> struct alignas(2 * sizeof(T)) pair_t { T a, b; };
 
+// cp.async of BYTES (4, 8 or 16) with zero fill: src_bytes = 0 writes zeros without touching global memory
+template <int BYTES> __device__ __forceinline__ void cp_async_zfill(void* smem, const void* gmem, int src_bytes)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;\n" ::"r"(s), "l"(gmem), "n"(BYTES), "r"(src_bytes));
+}
+
 template <typename T, bool MAP, bool MIXED>
 __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
 {
     extern __shared__ __align__(16) unsigned char lsm[];
-    T* tiles = reinterpret_cast<T*>(lsm);                                   // [4][3][k2Tile]
-    unsigned char* flags = lsm + (size_t)4 * 3 * k2Tile * sizeof(T);        // [4][k2Tile]
-    LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + 4 * k2Tile);   // [nmat]
+    // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
+    // three planes ahead of their use; with a map the loader goes through registers (vacuum cells are zeroed).
+    constexpr int NS = MAP ? 4 : 5;
+    T* tiles = reinterpret_cast<T*>(lsm);                                   // [NS][3][k2Tile]
+    unsigned char* flags = lsm + (size_t)NS * 3 * k2Tile * sizeof(T);       // [NS][k2Tile]
+    LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + NS * k2Tile);  // [nmat]
     unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
     using P2 = pair_t<T>;
 
@@ -405,8 +415,26 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
             }
         }
     };
+    auto slot_of = [&](int z) { return (int)((unsigned)(z - z0 + 1) % NS); };
+    auto async_plane = [&](int z) {
+        if (z > z1) { asm volatile("cp.async.commit_group;\n" ::); return; }     // not needed: empty group
+        int zz = z;
+        bool zin = true;
+        if (zz < 0 || zz >= nz) { if (a.periodic[2]) zz = ((zz % nz) + nz) % nz; else zin = false; }
+        const int64_t r0 = (int64_t)zz * nxy;
+        T* tl = tiles + slot_of(z) * 3 * k2Tile;
+#pragma unroll
+        for (int k = 0; k < k2NL; ++k) {
+            if (l_so[k] < 0) continue;
+            const bool ok = zin && l_go[k] >= 0;
+            const T* src = ok ? l_ptr[k] + r0 : Y;
+            if (l_pair[k]) cp_async_zfill<2 * (int)sizeof(T)>(tl + l_so[k], src, ok ? 2 * (int)sizeof(T) : 0);
+            else cp_async_zfill<(int)sizeof(T)>(tl + l_so[k], src, ok ? (int)sizeof(T) : 0);
+        }
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
     auto store_plane = [&](int z) {
-        const int slot = z & 3;
+        const int slot = slot_of(z);
         T* tl = tiles + slot * 3 * k2Tile;
         unsigned char* fl = flags + slot * k2Tile;
 #pragma unroll
@@ -422,11 +450,18 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
         }
     };
     __syncthreads();          // coefficient tables visible (fetch_plane reads sact)
-    fetch_plane(z0 - 1);
-    store_plane(z0 - 1);
-    fetch_plane(z0);
-    store_plane(z0);
-    fetch_plane(z0 + 1);
+    if (MAP) {
+        fetch_plane(z0 - 1);
+        store_plane(z0 - 1);
+        fetch_plane(z0);
+        store_plane(z0);
+        fetch_plane(z0 + 1);
+    } else {
+        async_plane(z0 - 1);
+        async_plane(z0);
+        async_plane(z0 + 1);
+        async_plane(z0 + 2);
+    }
 
     const int x = x0 + 2 * tx, y = y0 + ty;          // cells (x, y) and (x + 1, y)
     const bool inside = x < nx && y < ny;            // nx is even: both cells or none
@@ -455,9 +490,15 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
         for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + r);
     }
     for (int z = z0; z < z1; ++z) {
-        store_plane(z + 1);
-        __syncthreads();
-        if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
+        if (MAP) {
+            store_plane(z + 1);
+            __syncthreads();
+            if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
+        } else {
+            asm volatile("cp.async.wait_group 1;\n" ::);     // planes <= z+1 have landed
+            __syncthreads();
+            async_plane(z + 3);                              // into the slot of plane z-2 (commits a group)
+        }
         if (!inside) continue;
         const P2 ec[3] = {en[0], en[1], en[2]};
         if (Ee && z + 1 < z1) {
@@ -465,12 +506,13 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
 #pragma unroll
             for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + rn);
         }
-        const T* m0 = tiles + ((z - 1) & 3) * 3 * k2Tile;     // plane z-1
-        const T* c = tiles + (z & 3) * 3 * k2Tile;            // plane z
-        const T* p1 = tiles + ((z + 1) & 3) * 3 * k2Tile;     // plane z+1
-        const unsigned char* fm = flags + ((z - 1) & 3) * k2Tile;
-        const unsigned char* fc = flags + (z & 3) * k2Tile;
-        const unsigned char* fp = flags + ((z + 1) & 3) * k2Tile;
+        const int sm1 = slot_of(z - 1), s00 = slot_of(z), sp1 = slot_of(z + 1);
+        const T* m0 = tiles + sm1 * 3 * k2Tile;     // plane z-1
+        const T* c = tiles + s00 * 3 * k2Tile;      // plane z
+        const T* p1 = tiles + sp1 * 3 * k2Tile;     // plane z+1
+        const unsigned char* fm = flags + sm1 * k2Tile;
+        const unsigned char* fc = flags + s00 * k2Tile;
+        const unsigned char* fp = flags + sp1 * k2Tile;
         const int64_t r = (int64_t)z * nxy + rxy;
         const bool actA = !MAP || fc[c0], actB = !MAP || fc[c0 + 1];
         T EA[3] = {0, 0, 0}, EB[3] = {0, 0, 0};
@@ -596,7 +638,8 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
     a.zchunk = zc;
     dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
-    const size_t smem = two ? (size_t)4 * 3 * k2Tile * sizeof(T) + 4 * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1)
+    const int ns = a.map ? 4 : 5;         // ring slots of k_local2
+    const size_t smem = two ? (size_t)ns * 3 * k2Tile * sizeof(T) + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1)
                             : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
     static bool configured = false;
     if (!configured) {
