@@ -7,6 +7,7 @@
 //            zero outside the sample / in vacuum cells, c_ia = G11 (a == i) or G44 + G44', Gm = G12 + G44 - G44'
 //   then the integrator stage:  Yout = baseY + cy * k,  accOut = accIn + ca * k
 #include "fe_internal.h"
+#include <stdlib.h>
 
 namespace fe {
 
@@ -636,6 +637,7 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     // z chunk: as long as possible (halo planes are re-read per chunk) while the grid still fills the machine
     int zc = a.n[2];
     while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
+    if (getenv("FE_B200_ZC")) zc = atoi(getenv("FE_B200_ZC"));   // tuning aid
     a.zchunk = zc;
     dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
     const int ns = a.map ? 4 : 5;         // ring slots of k_local2
