@@ -133,6 +133,7 @@ def run_cuda(args):
     import torch
     import torch.distributed as dist
     import paper_2605_28800_b200 as fe
+    from paper_2605_28800_b200 import parallel as par
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -170,13 +171,9 @@ def run_cuda(args):
         g.step(P, w.dt, args.steps, fe.FE_EULER, fe.FE_TERM_ALL)
         ev1.record()
         barrier()
-    ms = ev0.elapsed_time(ev1)
     launches = g.launch_count() - l0
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = cells * world * args.steps / (ms * 1e-3)
+    # whole-job throughput: all ranks' cell-updates / the slowest rank's device time
+    value, ms = par.throughput(ev0.elapsed_time(ev1), float(cells * args.steps), device=dev)
     en = g.energy(P)[0]
 
     # ---- per-kernel durations, measured live with CUDA events on the launching stream (second pass of K steps)
@@ -217,13 +214,9 @@ def run_cuda(args):
         g.step(P, w.dt, 1, fe.FE_EULER, fe.FE_TERM_ALL)
         out_host.copy_(P, non_blocking=True)
         torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_value, _ = par.throughput((time.perf_counter() - t0) * 1e3, float(cells * e2e_steps), device=dev)
     nbytes = P_host.numel() * P_host.element_size()
-    e2e = {"value": cells * world * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes,
+    e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes,
            "d2h_bytes_per_step": nbytes, "steps": e2e_steps}
 
     # ---- cuFFT comparison (timed baseline, not the product): unpruned pad + rfftn + multiply + irfftn + crop
