@@ -174,3 +174,44 @@ def test_full_size_point_sources_against_closed_form(fe, cfg, dtype, tol):
     if w.batch > 1:
         assert float(g.rhs(P, fi.TERM_ELEC)[0].abs().max()) == 0.0      # other members untouched
     g.close()
+
+
+@pytest.mark.parametrize("n,periodic,images,dtype", [
+    ((64, 32, 32), (0, 0, 0), (0, 0, 0), "f64"),
+    ((128, 256, 128), (0, 0, 0), (0, 0, 0), "f64"),      # bulk-copy y pass (512), 256-point fused z pass
+    ((64, 128, 64), (0, 0, 0), (0, 0, 0), "f32"),        # bulk-copy y pass (256) in fp32
+    ((256, 128, 16), (1, 1, 0), (1, 1, 0), "f64"),       # unpruned x, y; generic z
+    ((16, 16, 8), (0, 0, 0), (0, 0, 0), "f64"),          # generic passes only
+])
+def test_no_write_outside_the_caller_buffers(fe, n, periodic, images, dtype):
+    """Guard bands around the workspace, the state and the output (compute-sanitizer is closed on the pool): every byte
+    outside the ranges the ABI documents must be untouched after precompute, rhs, step and energy."""
+    import torch
+    from paper_2605_28800_b200 import binding as bd
+    w = _workload(n, periodic, images)
+    g = fe.Grid.from_workload(w, dtype=dtype)
+    need, guard = bd.fe_workspace_bytes(g.h), 1 << 20
+    big = torch.full((need + 2 * guard,), 0xA5, dtype=torch.uint8, device="cuda:0")
+    ws = big[guard:guard + need]
+    assert ws.data_ptr() % 256 == 0
+    bd.fe_bind_workspace(g.h, ws)
+    g.ws = big
+    g.precompute_tensor()
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    numel = int(np.prod(g.state_shape))
+    pad = 4096
+    bufP = torch.full((numel + 2 * pad,), 7.0, dtype=tdt, device="cuda:0")
+    bufO = torch.full((numel + 2 * pad,), 7.0, dtype=tdt, device="cuda:0")
+    P = bufP[pad:pad + numel].view(g.state_shape)
+    O = bufO[pad:pad + numel].view(g.state_shape)
+    P.copy_(torch.from_numpy(w.P0).to(tdt))
+    bd.fe_rhs(g.h, P, O, fi.TERM_ALL)
+    g.step(P, w.dt, 3, fi.EULER, fi.TERM_ALL)
+    g.step(P, w.dt, 1, fi.RK4, fi.TERM_ALL)
+    g.energy(P)
+    torch.cuda.synchronize()
+    assert bool((big[:guard] == 0xA5).all()) and bool((big[guard + need:] == 0xA5).all())
+    for buf in (bufP, bufO):
+        assert bool((buf[:pad] == 7.0).all()) and bool((buf[pad + numel:] == 7.0).all())
+    assert bool(torch.isfinite(P).all()) and bool(torch.isfinite(O).all())
+    g.close()
