@@ -301,6 +301,25 @@ def config4_field_reduced(k: int) -> float:
     return _pto_units().field(config4_field(k))
 
 
+def landau_ensemble(temperatures: Sequence[float] = tuple(10.0 * j for j in range(37)),
+                    n: Tuple[int, int, int] = (16, 16, 8), seed: int = 1006) -> Workload:
+    """Landau-only ensemble (Fig. 2): one batch member per temperature
+    (T = 0 ... 360 K), every cell an independent single-cell relaxation (gradient, electrostatic and external terms
+    off) from a random orientation of magnitude 1e-3 C/m^2; 16x16x8 = 2048 starts per temperature
+    stand in for the paper's 1500.  Reduced units of BaTiO3 at 300 K for every member (the geometry is shared)."""
+    u = _bto_units()
+    nx, ny, nz = n
+    B = len(temperatures)
+    P = np.stack([sphere_uniform(np.random.default_rng(seed + b), (nz, ny, nx), 1e-3 / u.P0) for b in range(B)])
+    g = u.globals(Globals(**BATIO3_G, epsB=45.0))
+    h = u.length(1e-9)
+    return Workload(name=f"landau_ensemble_{B}T_{nx * ny * nz}starts", n=n, d=(h, h, h), periodic=(0, 0, 0),
+                    pbc_images=(0, 0, 0), batch=B, dtype="f64",
+                    materials=[[u.landau(batio3(float(T)))] for T in temperatures],
+                    globals_=[replace(g) for _ in range(B)], matmap=None, P0=P, dt=0.02, integrator=RK4,
+                    terms=TERM_LANDAU, nsteps=30000, notes="temperatures: " + ",".join("%g" % T for T in temperatures))
+
+
 def random_problem(seed: int, n=(6, 5, 4), periodic=(0, 1, 0), pbc_images=(0, 2, 0), n_materials: int = 3,
                    with_vacuum: bool = True, eighth: bool = True):
     """A small heterogeneous problem in O(1) units for the pins (P1, P9): random coefficients
