@@ -205,7 +205,7 @@ def run_cuda(args):
                 "kernels": kern}
 
     # ---- end to end through the C ABI with host buffers: H2D of the state, one step, D2H of the result ----
-    out_host = torch.empty_like(P_host)
+    out_host = torch.empty(P_host.shape, dtype=P_host.dtype, pin_memory=True)     # pinned: D2H at PCIe rate
     e2e_steps = max(1, min(args.steps, 5))
     barrier()
     t0 = time.perf_counter()

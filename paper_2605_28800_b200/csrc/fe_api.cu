@@ -65,6 +65,12 @@ struct fe_grid {
     bool tiled;                      // spectra and tensor table in the tiled layouts (all three passes fast)
     uint64_t launches;
     // optional per-kernel CUDA-event timing (fe_profile): event i precedes the launch of kind prof_kind[i]
+    // CUDA-graph replay of fe_step (one captured unit of steps, replayed on an internal stream)
+    cudaStream_t gstream;
+    cudaEvent_t gev_in, gev_out;
+    cudaGraphExec_t gexec;
+    bool gvalid, goff;               // cached graph usable / graphs disabled for this grid after a failure
+    void* gP; double gdt; int ginteg; uint32_t gterms; uint64_t gunit_launches;
     bool prof_on;
     std::vector<cudaEvent_t> prof_ev;
     std::vector<int> prof_kind;
@@ -232,6 +238,8 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     g->launches = 0;
     g->prof_on = false;
     g->prof_used = 0;
+    g->gstream = nullptr; g->gev_in = nullptr; g->gev_out = nullptr; g->gexec = nullptr;
+    g->gvalid = false; g->goff = false; g->gP = nullptr; g->gdt = 0.0; g->ginteg = -1; g->gterms = 0; g->gunit_launches = 0;
     const int B = d->batch, M = d->n_materials;
     g->h_mats.assign((size_t)B * M, DevLandau{});
     g->mat_set.assign((size_t)B * M, 0);
@@ -300,6 +308,10 @@ extern "C" fe_status fe_destroy_grid(fe_grid* g)
 {
     if (!g) return FE_OK;
     for (cudaEvent_t e : g->prof_ev) cudaEventDestroy(e);
+    if (g->gexec) cudaGraphExecDestroy(g->gexec);
+    if (g->gev_in) cudaEventDestroy(g->gev_in);
+    if (g->gev_out) cudaEventDestroy(g->gev_out);
+    if (g->gstream) cudaStreamDestroy(g->gstream);
     cudaFree(g->d_small);
     delete g;
     return FE_OK;
@@ -324,6 +336,7 @@ extern "C" fe_status fe_bind_workspace(fe_grid* g, void* dev, size_t bytes)
     g->ws = static_cast<unsigned char*>(dev);
     g->ws_bytes = bytes;
     g->tensor_ready = false;
+    g->gvalid = false;
     return FE_OK;
 }
 
@@ -390,6 +403,7 @@ extern "C" fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map)
 {
     if (!g) return fail(FE_EINVAL, "null argument");
     g->map = dev_map;
+    g->gvalid = false;
     return FE_OK;
 }
 
@@ -402,6 +416,7 @@ static fe_status sync_params(fe_grid* g, cudaStream_t st)
             if (!g->mat_set[(size_t)b * M + m]) return fail(FE_ESTATE, "material %d of member %d is unset", m, b);
     }
     if (!g->dirty) return FE_OK;
+    g->gvalid = false;               // kernel variants (mixed term) may change with the coefficients
     g->mixed = 0;
     for (int b = 0; b < B; ++b)
         if (g->h_members[b].Gm != 0.0) g->mixed = 1;
@@ -646,8 +661,61 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
     if (integ != FE_EULER && integ != FE_HEUN && integ != FE_RK4) return fail(FE_EINVAL, "unknown integrator");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = sync_params(g, st)) != FE_OK) return s;
-    s = g->f32 ? step_T<float>(g, (float*)P, dt, nsteps, integ, terms, st)
-               : step_T<double>(g, (double*)P, dt, nsteps, integ, terms, st);
+    auto run = [&](int n, cudaStream_t on) {
+        return g->f32 ? step_T<float>(g, (float*)P, dt, n, integ, terms, on) : step_T<double>(g, (double*)P, dt, n, integ, terms, on);
+    };
+    // Long runs replay a CUDA graph of one unit of steps (2 Euler steps: the ping-pong returns to P; 1 Heun / RK4 step)
+    // on an internal stream ordered with the caller's stream by events: small grids are launch bound otherwise.
+    // The first unit always runs eagerly (one-time kernel attribute set-up must not happen inside a capture).
+    const int unit = integ == FE_EULER ? 2 : 1;
+    static const bool graphs_off = getenv("FE_B200_GRAPH") && getenv("FE_B200_GRAPH")[0] == '0';
+    if (g->prof_on || g->goff || graphs_off || nsteps < 6 * unit) {
+        s = run(nsteps, st);
+        mark(g, -1, st);
+        return s;
+    }
+    if ((s = run(unit, st)) != FE_OK) return s;
+    int left = nsteps - unit;
+    const int reps = left / unit;
+    bool ok = true;
+    if (!g->gstream) {
+        ok = cudaStreamCreateWithFlags(&g->gstream, cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&g->gev_in, cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&g->gev_out, cudaEventDisableTiming) == cudaSuccess;
+    }
+    if (ok && !(g->gvalid && g->gP == P && g->gdt == dt && g->ginteg == integ && g->gterms == terms)) {
+        if (g->gexec) { cudaGraphExecDestroy(g->gexec); g->gexec = nullptr; }
+        g->gvalid = false;
+        cudaGraph_t graph = nullptr;
+        const uint64_t l0 = g->launches;
+        ok = cudaStreamBeginCapture(g->gstream, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+        if (ok) {
+            const fe_status cs = run(unit, g->gstream);
+            const cudaError_t ce = cudaStreamEndCapture(g->gstream, &graph);
+            ok = cs == FE_OK && ce == cudaSuccess && graph != nullptr;
+        }
+        g->gunit_launches = g->launches - l0;
+        g->launches = l0;                                   // the captured unit did not run
+        if (ok) ok = cudaGraphInstantiate(&g->gexec, graph, 0) == cudaSuccess;
+        if (graph) cudaGraphDestroy(graph);
+        if (ok) { g->gvalid = true; g->gP = P; g->gdt = dt; g->ginteg = integ; g->gterms = terms; }
+    }
+    if (ok) {
+        ok = cudaEventRecord(g->gev_in, st) == cudaSuccess && cudaStreamWaitEvent(g->gstream, g->gev_in, 0) == cudaSuccess;
+        for (int r = 0; ok && r < reps; ++r) ok = cudaGraphLaunch(g->gexec, g->gstream) == cudaSuccess;
+        if (ok) ok = cudaEventRecord(g->gev_out, g->gstream) == cudaSuccess && cudaStreamWaitEvent(st, g->gev_out, 0) == cudaSuccess;
+        if (ok) {
+            g->launches += (uint64_t)reps * g->gunit_launches;
+            left -= reps * unit;
+        } else {
+            return fail(FE_ECUDA, "CUDA graph replay failed: %s", cudaGetErrorString(cudaGetLastError()));
+        }
+    } else {
+        cudaGetLastError();                                 // capture unavailable: run eagerly from now on
+        g->goff = true;
+        g->gvalid = false;
+    }
+    s = left > 0 ? run(left, st) : FE_OK;
     mark(g, -1, st);
     return s;
 }

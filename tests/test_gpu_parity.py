@@ -215,3 +215,22 @@ def test_error_paths(fe):
     with pytest.raises(fe.FeError) as ei:           # material 1 unset
         g2.rhs(P, fi.TERM_LANDAU)
     assert ei.value.status == fe.FE_ESTATE
+
+
+@pytest.mark.parametrize("integ", [fi.EULER, fi.HEUN, fi.RK4])
+def test_graph_replay_equals_eager_stepping(fe, integ):
+    """fe_step(n) with n large replays a CUDA graph of one unit of steps; it must give bit-identical results to n single
+    eager steps, also after a coefficient change (graph invalidated) and with an odd number of Euler steps."""
+    w = workload_from_random(71, (8, 8, 4), (0, 1, 0), (0, 2, 0), batch=2)
+    g = _grid(fe, w)
+    for nsteps in (41, 64):
+        Pa, Pb = g.state(w.P0), g.state(w.P0)
+        g.step(Pa, 5e-3, nsteps, integ, fi.TERM_ALL)
+        for _ in range(nsteps):
+            g.step(Pb, 5e-3, 1, integ, fi.TERM_ALL)
+        assert np.array_equal(Pa.cpu().numpy(), Pb.cpu().numpy())
+        g.set_external_field(0, (0.01 * nsteps, 0.0, -0.02))          # invalidates the cached graph
+    o = orc.Oracle(oracle_problem(w, 1), elec="direct")
+    Pc = g.state(w.P0)
+    g.step(Pc, 5e-3, 30, integ, fi.TERM_ALL)
+    assert rel_l2(Pc.cpu().numpy()[1], o.step(w.P0[1], 5e-3, 30, integ, fi.TERM_ALL)) < 1e-11
