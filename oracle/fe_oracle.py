@@ -252,6 +252,18 @@ def field_fft(p: Problem, K: np.ndarray, P: np.ndarray, box_hat: Optional[np.nda
 
 
 # ---------------------------------------------------------------- O5-O7
+# Cash-Karp tableau (Cash & Karp 1990): a_ij, 5th-order weights, embedded 4th-order weights
+RK45_C = (0.0, 1.0 / 5.0, 3.0 / 10.0, 3.0 / 5.0, 1.0, 7.0 / 8.0)
+RK45_A = ((),
+          (1.0 / 5.0,),
+          (3.0 / 40.0, 9.0 / 40.0),
+          (3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0),
+          (-11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0),
+          (1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0))
+RK45_B5 = (37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0)
+RK45_B4 = (2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0, 277.0 / 14336.0, 1.0 / 4.0)
+
+
 class Oracle:
     """RHS / step / energy of one simulation.  elec = 'direct' (O3) or 'fft' (O8)."""
 
@@ -308,6 +320,65 @@ class Oracle:
             else:
                 raise ValueError("integrator")
         return P
+
+    def step_ab3m2(self, P: np.ndarray, dt: float, nsteps: int, terms: int = TERM_ALL) -> np.ndarray:
+        """AB3M2 ("Adams-Bashforth (AB3M2), a multistep explicit scheme", ref. [53]), reading A18:
+        predictor = 3-step Adams-Bashforth, corrector = 2nd-order Adams-Moulton (trapezoid), one correction (PECE);
+        the first two steps, which have no history, are Heun steps:
+            P*      = P_n + dt/12 (23 f_n - 16 f_{n-1} + 5 f_{n-2})
+            P_{n+1} = P_n + dt/2  (f_n + f(P*))"""
+        P = np.array(P, dtype=np.float64, copy=True)
+        f = lambda Y: self.rhs(Y, terms)
+        hist = []                                    # f_{n-1}, f_{n-2}
+        for n in range(nsteps):
+            fn = f(P)
+            if n < 2:
+                Pstar = P + dt * fn
+            else:
+                Pstar = P + (dt / 12.0) * (23.0 * fn - 16.0 * hist[0] + 5.0 * hist[1])
+            P = P + (dt / 2.0) * (fn + f(Pstar))
+            hist = [fn] + hist[:1]
+        return P
+
+    def step_rk45(self, P: np.ndarray, t_span: float, dt_init: float, tol: float, max_steps: int = 100000,
+                  terms: int = TERM_ALL):
+        """Adaptive RK45 (ref. [52] "fifth order Runge-Kutta with adaptive step size control"), reading
+        A17: the Cash-Karp embedded pair; the 5th-order solution is propagated, err = max over cells and components
+        of |y5 - y4| / tol (absolute tolerance, state units); a step is accepted when err <= 1,
+            accepted: dt_next = 0.9 dt err^-0.2  (5 dt when err <= 1.89e-4),
+            rejected: dt      = max(0.9 dt err^-0.25, 0.1 dt);
+        the last step is shortened to land on t_span.  Returns (P, stats)."""
+        P = np.array(P, dtype=np.float64, copy=True)
+        f = lambda Y: self.rhs(Y, terms)
+        A, B5, B4 = RK45_A, RK45_B5, RK45_B4
+        t, dt = 0.0, float(dt_init)
+        acc = rej = evals = 0
+        err = 0.0
+        dt_last = 0.0
+        while t < t_span and acc + rej < max_steps:
+            h = min(dt, t_span - t)
+            k = []
+            for i in range(6):
+                Y = P.copy()
+                for j in range(i):
+                    if A[i][j] != 0.0:
+                        Y = Y + (h * A[i][j]) * k[j]
+                k.append(f(Y))
+            evals += 6
+            y5 = P.copy()
+            d = np.zeros_like(P)
+            for j in range(6):
+                if B5[j] != 0.0:
+                    y5 = y5 + (h * B5[j]) * k[j]
+                d = d + (h * (B5[j] - B4[j])) * k[j]
+            err = float(np.max(np.abs(d))) / tol
+            if err <= 1.0:
+                P, t, acc, dt_last = y5, t + h, acc + 1, h
+                dt = 5.0 * h if err <= 1.89e-4 else 0.9 * h * err ** -0.2
+            else:
+                rej += 1
+                dt = max(0.9 * h * err ** -0.25, 0.1 * h)
+        return P, dict(t=t, accepted=acc, rejected=rej, rhs_evals=evals, dt_last=dt_last, dt_next=dt, err_last=err)
 
     def energy(self, P: np.ndarray, terms: int = TERM_ALL) -> np.ndarray:
         """[F_Land, F_Grad, F_Elec, F_Ext, F_tot, <Px>, <Py>, <Pz>] (means over active cells)."""
