@@ -20,7 +20,7 @@ import numpy as np
 EPS0_SI = 8.8541878128e-12
 
 TERM_LANDAU, TERM_GRADIENT, TERM_ELEC, TERM_EXT, TERM_ALL = 1, 2, 4, 8, 15
-EULER, HEUN, RK4 = 0, 1, 2
+EULER, HEUN, RK4, AB3M2 = 0, 1, 2, 3
 
 
 # --------------------------------------------------------------------------------------

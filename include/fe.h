@@ -47,7 +47,9 @@ typedef enum {
 
 enum { FE_F64 = 0, FE_F32 = 1 };
 enum { FE_TERM_LANDAU = 1, FE_TERM_GRADIENT = 2, FE_TERM_ELEC = 4, FE_TERM_EXT = 8, FE_TERM_ALL = 15 };
-enum { FE_EULER = 0, FE_HEUN = 1, FE_RK4 = 2 };   /* PAPER.md:117-119; RK4 = BASELINE.json config 2 */
+enum { FE_EULER = 0, FE_HEUN = 1, FE_RK4 = 2,     /* PAPER.md:117-119; RK4 = BASELINE.json config 2 */
+       FE_AB3M2 = 3 };   /* 3-step Adams-Bashforth predictor + 2nd-order Adams-Moulton corrector (PECE),
+                            the first two steps of a call are Heun steps (reading A18) */
 
 /* Geometry of the batch (PAPER.md:113 uniform cells; PAPER.md:117 batch). */
 typedef struct {
@@ -103,6 +105,23 @@ fe_status fe_rhs(fe_grid* g, const void* P, void* dPdt, uint32_t terms, void* cu
  * the call. */
 fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int32_t integrator,
                   uint32_t terms, void* cuda_stream);
+
+/* Adaptive RK45 (ref. [52]; reading A17): Cash-Karp embedded pair, the 5th-order solution
+ * is propagated over t_span starting with step dt_init; err = max over all cells, components and batch members of
+ * |y5 - y4| / tol (tol: absolute, in the units of P); a step is accepted when err <= 1, then
+ * dt_next = 0.9 dt err^-0.2 (5 dt when err <= 1.89e-4), else dt = max(0.9 dt err^-0.25, 0.1 dt) and the step is
+ * retried; the last step is shortened to land on t_span.  All batch members advance with the same step.  At most
+ * max_steps attempts are made (stats->t < t_span then).  Synchronises the stream once per attempt (the decision
+ * is taken on the host); *stats is HOST memory and may be NULL.  Needs the workspace of fe_workspace_bytes. */
+typedef struct {
+    double t;            /* time reached */
+    double dt_last;      /* size of the last accepted step */
+    double dt_next;      /* step the controller proposes next */
+    double err_last;     /* scaled error of the last attempt */
+    int32_t accepted, rejected, rhs_evals;
+} fe_rk45_stats;
+fe_status fe_step_rk45(fe_grid* g, void* P, double t_span, double dt_init, double tol, int32_t max_steps,
+                       uint32_t terms, fe_rk45_stats* stats, void* cuda_stream);
 
 /* a6: host_out[b][8] = { F_Land, F_Grad, F_Elec, F_Ext, F_tot, <Px>, <Py>, <Pz> } for the terms in
  * the bitmask (Eq. 2, 5, 7); energies are densities times cell volume summed over cells, means are

@@ -18,13 +18,19 @@ from . import build as _build
 FE_OK, FE_EINVAL, FE_ENOMEM, FE_ECUDA, FE_ESTATE, FE_ENONFINITE = range(6)
 FE_F64, FE_F32 = 0, 1
 FE_TERM_LANDAU, FE_TERM_GRADIENT, FE_TERM_ELEC, FE_TERM_EXT, FE_TERM_ALL = 1, 2, 4, 8, 15
-FE_EULER, FE_HEUN, FE_RK4 = 0, 1, 2
+FE_EULER, FE_HEUN, FE_RK4, FE_AB3M2 = 0, 1, 2, 3
 
 SYMBOLS = ["fe_create_grid", "fe_destroy_grid", "fe_workspace_bytes", "fe_bind_workspace", "fe_set_material",
            "fe_set_global", "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs",
            "fe_step", "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_launch_count", "fe_last_error",
-           "fe_version", "fe_profile", "fe_profile_read"]
+           "fe_version", "fe_profile", "fe_profile_read", "fe_step_rk45"]
 KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other"]
+
+
+class fe_rk45_stats(ctypes.Structure):
+    _fields_ = [("t", ctypes.c_double), ("dt_last", ctypes.c_double), ("dt_next", ctypes.c_double),
+                ("err_last", ctypes.c_double), ("accepted", ctypes.c_int32), ("rejected", ctypes.c_int32),
+                ("rhs_evals", ctypes.c_int32)]
 
 
 class fe_grid_desc(ctypes.Structure):
@@ -85,6 +91,7 @@ def load():
         L.fe_profile.argtypes = [vp, i32]
         L.fe_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_uint64), vp]
         L.fe_launch_count.argtypes = [vp]
+        L.fe_step_rk45.argtypes = [vp, vp, dbl, dbl, dbl, i32, u32, ctypes.POINTER(fe_rk45_stats), vp]
         L.fe_launch_count.restype = ctypes.c_uint64
         L.fe_last_error.restype = ctypes.c_char_p
         L.fe_version.restype = ctypes.c_char_p
@@ -171,6 +178,15 @@ def fe_rhs(h, P: torch.Tensor, dPdt: torch.Tensor, terms: int = FE_TERM_ALL):
 
 def fe_step(h, P: torch.Tensor, dt: float, nsteps: int, integrator: int = FE_EULER, terms: int = FE_TERM_ALL):
     _check(load().fe_step(h, ctypes.c_void_p(P.data_ptr()), float(dt), int(nsteps), int(integrator), terms, _stream()))
+
+
+def fe_step_rk45(h, P: torch.Tensor, t_span: float, dt_init: float, tol: float, max_steps: int = 100000,
+                 terms: int = FE_TERM_ALL) -> dict:
+    st = fe_rk45_stats()
+    _check(load().fe_step_rk45(h, ctypes.c_void_p(P.data_ptr()), float(t_span), float(dt_init), float(tol), int(max_steps),
+                               terms, ctypes.byref(st), _stream()))
+    return dict(t=st.t, dt_last=st.dt_last, dt_next=st.dt_next, err_last=st.err_last, accepted=st.accepted,
+                rejected=st.rejected, rhs_evals=st.rhs_evals)
 
 
 def fe_energy(h, P: torch.Tensor, batch: int, terms: int = FE_TERM_ALL, allow_nonfinite: bool = False) -> np.ndarray:
@@ -265,6 +281,9 @@ class Grid:
     def step(self, P: torch.Tensor, dt, nsteps, integrator=FE_EULER, terms=FE_TERM_ALL):
         fe_step(self.h, P, dt, nsteps, integrator, terms)
         return P
+
+    def step_rk45(self, P: torch.Tensor, t_span, dt_init, tol, max_steps=100000, terms=FE_TERM_ALL) -> dict:
+        return fe_step_rk45(self.h, P, t_span, dt_init, tol, max_steps, terms)
 
     def energy(self, P: torch.Tensor, terms=FE_TERM_ALL, allow_nonfinite=False) -> np.ndarray:
         return fe_energy(self.h, P, self.batch, terms, allow_nonfinite)

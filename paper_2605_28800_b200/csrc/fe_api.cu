@@ -58,7 +58,7 @@ struct fe_grid {
     // workspace (borrowed)
     unsigned char* ws;
     size_t ws_bytes;
-    size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_part, o_box, o_Sbox, total_bytes;
+    size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_K[6], o_part, o_box, o_Sbox, total_bytes;
     int nblk;
     bool tensor_ready;
     bool fast[3];                    // size-specialised register FFT kernels available for the x / y / z pass
@@ -156,6 +156,7 @@ static void layout_workspace(fe_grid* g)
     g->o_Y = off;   off += align_up((size_t)B * 3 * g->N * g->rsz);
     g->o_ACC = off; off += align_up((size_t)B * 3 * g->N * g->rsz);
     g->o_PP = off;  off += align_up((size_t)B * 3 * g->N * g->rsz);
+    for (int j = 0; j < 6; ++j) { g->o_K[j] = off; off += align_up((size_t)B * 3 * g->N * g->rsz); }   // RK45 / AB3M2 stages
     const size_t hot1 = off;
     // precompute scratch overlays the hot region (the tensor is computed before any step)
     size_t s = hot0;
@@ -640,6 +641,34 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
             if ((s = stage<T>(g, P, P, Y, dt, P, ACC, 0.5 * dt, terms, st)) != FE_OK) return s;
             if ((s = stage<T>(g, Y, ACC, P, 0.5 * dt, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
         }
+    } else if (integ == FE_AB3M2) {
+        // P* = P + dt/12 (23 f_n - 16 f_{n-1} + 5 f_{n-2}) (Euler predictor while there is no history),
+        // P <- P + dt/2 (f_n + f(P*)); the history restarts with every call
+        T* F[3] = {reinterpret_cast<T*>(g->ws + g->o_K[0]), reinterpret_cast<T*>(g->ws + g->o_K[1]),
+                   reinterpret_cast<T*>(g->ws + g->o_K[2])};
+        T* FS = reinterpret_cast<T*>(g->ws + g->o_K[3]);
+        const int64_t n = (int64_t)g->desc.batch * 3 * g->N;
+        for (int i = 0; i < nsteps; ++i) {
+            if ((s = stage<T>(g, P, nullptr, F[0], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+            LinArgs a;
+            memset(&a, 0, sizeof(a));
+            if (i < 2) {
+                a.k[0] = F[0]; a.c[0] = dt;
+                FE_CUDA(launch_lincomb<T>(Y, P, a, 1, n, st));
+            } else {
+                a.k[0] = F[0]; a.c[0] = dt * 23.0 / 12.0;
+                a.k[1] = F[1]; a.c[1] = -dt * 16.0 / 12.0;
+                a.k[2] = F[2]; a.c[2] = dt * 5.0 / 12.0;
+                FE_CUDA(launch_lincomb<T>(Y, P, a, 3, n, st));
+            }
+            if ((s = stage<T>(g, Y, nullptr, FS, 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+            memset(&a, 0, sizeof(a));
+            a.k[0] = F[0]; a.c[0] = 0.5 * dt;
+            a.k[1] = FS;   a.c[1] = 0.5 * dt;
+            FE_CUDA(launch_lincomb<T>(P, P, a, 2, n, st));
+            g->launches += 2;
+            T* t = F[2]; F[2] = F[1]; F[1] = F[0]; F[0] = t;
+        }
     } else {
         for (int i = 0; i < nsteps; ++i) {
             // classical RK4, weights 1/6 1/3 1/3 1/6, stage points P + dt/2 k1, P + dt/2 k2, P + dt k3
@@ -658,7 +687,7 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
     if (s != FE_OK) return s;
     if (nsteps < 0) return fail(FE_EINVAL, "nsteps < 0");
     if (!isfinite(dt)) return fail(FE_EINVAL, "dt not finite");
-    if (integ != FE_EULER && integ != FE_HEUN && integ != FE_RK4) return fail(FE_EINVAL, "unknown integrator");
+    if (integ != FE_EULER && integ != FE_HEUN && integ != FE_RK4 && integ != FE_AB3M2) return fail(FE_EINVAL, "unknown integrator");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = sync_params(g, st)) != FE_OK) return s;
     auto run = [&](int n, cudaStream_t on) {
@@ -669,7 +698,7 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
     // The first unit always runs eagerly (one-time kernel attribute set-up must not happen inside a capture).
     const int unit = integ == FE_EULER ? 2 : 1;
     static const bool graphs_off = getenv("FE_B200_GRAPH") && getenv("FE_B200_GRAPH")[0] == '0';
-    if (g->prof_on || g->goff || graphs_off || nsteps < 6 * unit) {
+    if (g->prof_on || g->goff || graphs_off || nsteps < 6 * unit || integ == FE_AB3M2) {
         s = run(nsteps, st);
         mark(g, -1, st);
         return s;
@@ -716,6 +745,85 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
         g->gvalid = false;
     }
     s = left > 0 ? run(left, st) : FE_OK;
+    mark(g, -1, st);
+    return s;
+}
+
+// ---- adaptive Cash-Karp RK45 (include/fe.h states the controller) ----------------
+template <typename T>
+static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double tol, int max_steps, uint32_t terms,
+                        fe_rk45_stats* out, cudaStream_t st)
+{
+    static const double A[6][5] = {{0, 0, 0, 0, 0},
+                                   {1.0 / 5.0, 0, 0, 0, 0},
+                                   {3.0 / 40.0, 9.0 / 40.0, 0, 0, 0},
+                                   {3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0, 0, 0},
+                                   {-11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0, 0},
+                                   {1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0}};
+    static const double B5[6] = {37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0};
+    static const double B4[6] = {2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0, 277.0 / 14336.0, 1.0 / 4.0};
+    T* K[6];
+    for (int j = 0; j < 6; ++j) K[j] = reinterpret_cast<T*>(g->ws + g->o_K[j]);
+    T* Y = reinterpret_cast<T*>(g->ws + g->o_Y);
+    T* Y5 = reinterpret_cast<T*>(g->ws + g->o_PP);
+    const int64_t n = (int64_t)g->desc.batch * 3 * g->N;
+    const size_t bytes = (size_t)n * sizeof(T);
+    double t = 0.0, dt = dt_init, err = 0.0, dt_last = 0.0;
+    int acc = 0, rej = 0, evals = 0;
+    fe_status s;
+    while (t < t_span && acc + rej < max_steps) {
+        const double h = dt < t_span - t ? dt : t_span - t;
+        for (int i = 0; i < 6; ++i) {
+            const T* Yi = P;
+            if (i > 0) {
+                LinArgs a;
+                memset(&a, 0, sizeof(a));
+                int nk = 0;
+                for (int j = 0; j < i; ++j)
+                    if (A[i][j] != 0.0) { a.k[nk] = K[j]; a.c[nk] = h * A[i][j]; ++nk; }
+                FE_CUDA(launch_lincomb<T>(Y, P, a, nk, n, st));
+                g->launches += 1;
+                Yi = Y;
+            }
+            if ((s = stage<T>(g, Yi, nullptr, K[i], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+        }
+        evals += 6;
+        LinArgs b5, d;
+        for (int j = 0; j < 6; ++j) { b5.k[j] = d.k[j] = K[j]; b5.c[j] = h * B5[j]; d.c[j] = h * (B5[j] - B4[j]); }
+        FE_CUDA(launch_rk45_final<T>(Y5, P, b5, d, n, g->d_eout, st));
+        g->launches += 1;
+        double emax = 0.0;
+        FE_CUDA(cudaMemcpyAsync(&emax, g->d_eout, sizeof(double), cudaMemcpyDeviceToHost, st));
+        FE_CUDA(cudaStreamSynchronize(st));
+        err = emax / tol;
+        if (err <= 1.0) {                                // NaN compares false: a non-finite estimate rejects
+            FE_CUDA(cudaMemcpyAsync(P, Y5, bytes, cudaMemcpyDeviceToDevice, st));
+            t += h; ++acc; dt_last = h;
+            dt = err <= 1.89e-4 ? 5.0 * h : 0.9 * h * pow(err, -0.2);
+        } else {
+            ++rej;
+            const double shr = 0.9 * h * pow(err, -0.25);
+            dt = (shr > 0.1 * h) ? shr : 0.1 * h;         // also taken when err is NaN
+            if (!isfinite(err) && rej > 60) return fail(FE_ENONFINITE, "RK45: non-finite error estimate");
+        }
+    }
+    FE_CUDA(cudaStreamSynchronize(st));
+    if (out) { out->t = t; out->dt_last = dt_last; out->dt_next = dt; out->err_last = err;
+               out->accepted = acc; out->rejected = rej; out->rhs_evals = evals; }
+    return FE_OK;
+}
+
+extern "C" fe_status fe_step_rk45(fe_grid* g, void* P, double t_span, double dt_init, double tol, int32_t max_steps,
+                                  uint32_t terms, fe_rk45_stats* stats, void* stream)
+{
+    fe_status s = check_ready(g, P, terms);
+    if (s != FE_OK) return s;
+    if (!(t_span >= 0.0) || !(dt_init > 0.0) || !(tol > 0.0) || !isfinite(t_span) || !isfinite(dt_init) || max_steps < 0)
+        return fail(FE_EINVAL, "RK45: t_span >= 0, dt_init > 0, tol > 0, max_steps >= 0 required");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((s = sync_params(g, st)) != FE_OK) return s;
+    s = g->f32 ? rk45_T<float>(g, (float*)P, t_span, dt_init, tol, max_steps, terms, stats, st)
+               : rk45_T<double>(g, (double*)P, t_span, dt_init, tol, max_steps, terms, stats, st);
     mark(g, -1, st);
     return s;
 }

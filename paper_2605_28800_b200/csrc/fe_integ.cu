@@ -1,0 +1,79 @@
+// fe_integ.cu -- array kernels of the multistep / adaptive integrators:
+//   k_lincomb     out = base + sum_j c_j k_j                      (stage states of RK45, predictor / corrector of AB3M2)
+//   k_rk45_final  y5 = P + sum_j b5_j k_j,  err = max |sum_j d_j k_j|   (Cash-Karp 5th-order solution + embedded error)
+// Plain streaming passes (HBM bound); the right-hand sides themselves come from the fused local step (fe_local.cu).
+#include "fe_internal.h"
+
+namespace fe {
+
+template <typename T, int NK>
+__global__ void __launch_bounds__(256) k_lincomb(T* __restrict__ out, const T* __restrict__ base, LinArgs a, int64_t n)
+{
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        T v = base[i];
+#pragma unroll
+        for (int j = 0; j < NK; ++j) v = v + (T)a.c[j] * static_cast<const T*>(a.k[j])[i];
+        out[i] = v;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_rk45_final(T* __restrict__ y5, const T* __restrict__ P, LinArgs b5, LinArgs d,
+                                                    int64_t n, unsigned long long* __restrict__ err_bits)
+{
+    double m = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        T v = P[i], e = (T)0;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            const T kj = static_cast<const T*>(b5.k[j])[i];
+            if (b5.c[j] != 0.0) v = v + (T)b5.c[j] * kj;
+            e = e + (T)d.c[j] * kj;
+        }
+        y5[i] = v;
+        m = fmax(m, fabs((double)e));
+    }
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+    __shared__ double red[8];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) red[warp] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, red[w]);
+        // non-negative doubles order like their bit patterns; NaN (all-ones exponent, non-zero mantissa) sorts above
+        // +inf, so a non-finite error estimate always rejects the step
+        atomicMax(err_bits, (unsigned long long)__double_as_longlong(m));
+    }
+}
+
+template <typename T>
+cudaError_t launch_lincomb(T* out, const T* base, const LinArgs& a, int nk, int64_t n, cudaStream_t st)
+{
+    const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    switch (nk) {
+        case 1: k_lincomb<T, 1><<<grid, 256, 0, st>>>(out, base, a, n); break;
+        case 2: k_lincomb<T, 2><<<grid, 256, 0, st>>>(out, base, a, n); break;
+        case 3: k_lincomb<T, 3><<<grid, 256, 0, st>>>(out, base, a, n); break;
+        case 4: k_lincomb<T, 4><<<grid, 256, 0, st>>>(out, base, a, n); break;
+        case 5: k_lincomb<T, 5><<<grid, 256, 0, st>>>(out, base, a, n); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_rk45_final(T* y5, const T* P, const LinArgs& b5, const LinArgs& d, int64_t n, double* err, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(err, 0, sizeof(double), st);
+    if (e != cudaSuccess) return e;
+    const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
+    k_rk45_final<T><<<grid, 256, 0, st>>>(y5, P, b5, d, n, reinterpret_cast<unsigned long long*>(err));
+    return cudaGetLastError();
+}
+
+template cudaError_t launch_lincomb<double>(double*, const double*, const LinArgs&, int, int64_t, cudaStream_t);
+template cudaError_t launch_lincomb<float>(float*, const float*, const LinArgs&, int, int64_t, cudaStream_t);
+template cudaError_t launch_rk45_final<double>(double*, const double*, const LinArgs&, const LinArgs&, int64_t, double*, cudaStream_t);
+template cudaError_t launch_rk45_final<float>(float*, const float*, const LinArgs&, const LinArgs&, int64_t, double*, cudaStream_t);
+
+}  // namespace fe

@@ -169,4 +169,16 @@ struct EnergyArgs {
 };
 template <typename T> cudaError_t launch_energy(const EnergyArgs& a, cudaStream_t st);
 
+// ---- integrator array kernels (fe_integ.cu) ---------------------------------------------------
+struct LinArgs {
+    const void* k[6];
+    double c[6];
+};
+// out = base + sum_{j < nk} c_j k_j   (nk in 1..5; out may alias base)
+template <typename T>
+cudaError_t launch_lincomb(T* out, const T* base, const LinArgs& a, int nk, int64_t n, cudaStream_t st);
+// y5 = P + sum_j b5.c_j k_j;  *err (device double, reset here) = max_i |sum_j d.c_j k_j[i]|
+template <typename T>
+cudaError_t launch_rk45_final(T* y5, const T* P, const LinArgs& b5, const LinArgs& d, int64_t n, double* err, cudaStream_t st);
+
 }  // namespace fe
