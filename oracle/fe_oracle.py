@@ -17,6 +17,7 @@ direct sum in tests/test_oracle_electrostatics.py and used where O(N^2) is too s
 from __future__ import annotations
 
 import ctypes
+import math
 import os
 import subprocess
 from dataclasses import dataclass, field
@@ -272,6 +273,18 @@ class Oracle:
         self.elec = elec
         self.K = K
         self._box_hat = None
+        self.wave = None        # (amp[3], omega, phase): E_ext(t) = g.E_ext + amp sin(omega t + phase)
+
+    def set_wave(self, amp, omega: float, phase: float = 0.0):
+        """Time-dependent external excitation: a sinusoid added to the static field."""
+        self.wave = (np.array(amp, dtype=np.float64), float(omega), float(phase))
+
+    def e_ext(self, t: float = 0.0) -> np.ndarray:
+        E = np.array(self.p.g.E_ext, dtype=np.float64)
+        if self.wave is not None:
+            amp, om, ph = self.wave
+            E = E + amp * math.sin(om * t + ph)
+        return E
 
     def table(self) -> np.ndarray:
         if self.K is None:
@@ -286,62 +299,65 @@ class Oracle:
             self._box_hat = np.fft.fftn(circular_kernel(self.p, K), axes=(1, 2, 3))
         return field_fft(self.p, K, P, self._box_hat)
 
-    def fields(self, P: np.ndarray, terms: int = TERM_ALL):
+    def fields(self, P: np.ndarray, terms: int = TERM_ALL, t: float = 0.0):
         p = self.p
         z = np.zeros(p.shape)
         El = landau_field(p, P) if terms & TERM_LANDAU else z
         Eg = grad_field(p, P) if terms & TERM_GRADIENT else z
         Ee = self.elec_field(P) if terms & TERM_ELEC else z
-        Ex = (np.array(p.g.E_ext, dtype=np.float64)[:, None, None, None] * np.ones(p.shape)
+        Ex = (self.e_ext(t)[:, None, None, None] * np.ones(p.shape)
               if terms & TERM_EXT else z)
         return El, Eg, Ee, Ex
 
-    def rhs(self, P: np.ndarray, terms: int = TERM_ALL) -> np.ndarray:
-        El, Eg, Ee, Ex = self.fields(P, terms)
+    def rhs(self, P: np.ndarray, terms: int = TERM_ALL, t: float = 0.0) -> np.ndarray:
+        El, Eg, Ee, Ex = self.fields(P, terms, t)
         return self.p.g.L * self.p.active[None] * (El + Eg + Ee + Ex)
 
     def step(self, P: np.ndarray, dt: float, nsteps: int = 1, integrator: int = EULER,
-             terms: int = TERM_ALL) -> np.ndarray:
+             terms: int = TERM_ALL, t0: float = 0.0) -> np.ndarray:
+        """Step n goes from t0 + n dt to t0 + (n + 1) dt; the stages sample E_ext at the usual abscissae."""
         P = np.array(P, dtype=np.float64, copy=True)
-        f = lambda Y: self.rhs(Y, terms)
-        for _ in range(nsteps):
+        f = lambda Y, t: self.rhs(Y, terms, t)
+        for n in range(nsteps):
+            t = t0 + n * dt
             if integrator == EULER:
-                P = P + dt * f(P)
+                P = P + dt * f(P, t)
             elif integrator == HEUN:
-                k1 = f(P)
-                k2 = f(P + dt * k1)
+                k1 = f(P, t)
+                k2 = f(P + dt * k1, t + dt)
                 P = P + (dt / 2.0) * (k1 + k2)
             elif integrator == RK4:
-                k1 = f(P)
-                k2 = f(P + (dt / 2.0) * k1)
-                k3 = f(P + (dt / 2.0) * k2)
-                k4 = f(P + dt * k3)
+                k1 = f(P, t)
+                k2 = f(P + (dt / 2.0) * k1, t + dt / 2.0)
+                k3 = f(P + (dt / 2.0) * k2, t + dt / 2.0)
+                k4 = f(P + dt * k3, t + dt)
                 P = P + dt * (k1 / 6.0 + k2 / 3.0 + k3 / 3.0 + k4 / 6.0)
             else:
                 raise ValueError("integrator")
         return P
 
-    def step_ab3m2(self, P: np.ndarray, dt: float, nsteps: int, terms: int = TERM_ALL) -> np.ndarray:
+    def step_ab3m2(self, P: np.ndarray, dt: float, nsteps: int, terms: int = TERM_ALL, t0: float = 0.0) -> np.ndarray:
         """AB3M2 ("Adams-Bashforth (AB3M2), a multistep explicit scheme", ref. [53]), reading A18:
         predictor = 3-step Adams-Bashforth, corrector = 2nd-order Adams-Moulton (trapezoid), one correction (PECE);
         the first two steps, which have no history, are Heun steps:
             P*      = P_n + dt/12 (23 f_n - 16 f_{n-1} + 5 f_{n-2})
             P_{n+1} = P_n + dt/2  (f_n + f(P*))"""
         P = np.array(P, dtype=np.float64, copy=True)
-        f = lambda Y: self.rhs(Y, terms)
+        f = lambda Y, t: self.rhs(Y, terms, t)
         hist = []                                    # f_{n-1}, f_{n-2}
         for n in range(nsteps):
-            fn = f(P)
+            t = t0 + n * dt
+            fn = f(P, t)
             if n < 2:
                 Pstar = P + dt * fn
             else:
                 Pstar = P + (dt / 12.0) * (23.0 * fn - 16.0 * hist[0] + 5.0 * hist[1])
-            P = P + (dt / 2.0) * (fn + f(Pstar))
+            P = P + (dt / 2.0) * (fn + f(Pstar, t + dt))
             hist = [fn] + hist[:1]
         return P
 
     def step_rk45(self, P: np.ndarray, t_span: float, dt_init: float, tol: float, max_steps: int = 100000,
-                  terms: int = TERM_ALL):
+                  terms: int = TERM_ALL, t0: float = 0.0):
         """Adaptive RK45 (ref. [52] "fifth order Runge-Kutta with adaptive step size control"), reading
         A17: the Cash-Karp embedded pair; the 5th-order solution is propagated, err = max over cells and components
         of |y5 - y4| / tol (absolute tolerance, state units); a step is accepted when err <= 1,
@@ -349,8 +365,8 @@ class Oracle:
             rejected: dt      = max(0.9 dt err^-0.25, 0.1 dt);
         the last step is shortened to land on t_span.  Returns (P, stats)."""
         P = np.array(P, dtype=np.float64, copy=True)
-        f = lambda Y: self.rhs(Y, terms)
-        A, B5, B4 = RK45_A, RK45_B5, RK45_B4
+        f = lambda Y, tt: self.rhs(Y, terms, tt)
+        A, B5, B4, C = RK45_A, RK45_B5, RK45_B4, RK45_C
         t, dt = 0.0, float(dt_init)
         acc = rej = evals = 0
         err = 0.0
@@ -363,7 +379,7 @@ class Oracle:
                 for j in range(i):
                     if A[i][j] != 0.0:
                         Y = Y + (h * A[i][j]) * k[j]
-                k.append(f(Y))
+                k.append(f(Y, t0 + t + C[i] * h))
             evals += 6
             y5 = P.copy()
             d = np.zeros_like(P)

@@ -95,3 +95,47 @@ def test_rk45_controller_meets_the_tolerance_and_lands_on_t_span():
     # max_steps bounds the work
     P, st = o.step_rk45(P0, 3.0, 1e-3, 1e-12, 7, orc.TERM_LANDAU)
     assert st["accepted"] + st["rejected"] == 7 and st["t"] < 3.0
+
+
+def _forced_problem():
+    """One cell, dP_z/dt = -lam P_z + A sin(om t) (Landau a1 > 0 + sinusoidal external field):
+    P(t) = exp(-lam t) P0 + A [lam sin(om t) - om cos(om t) + om exp(-lam t)] / (lam^2 + om^2)."""
+    m = fi.Landau(a1=(0.7, 1.1, 0.4))
+    p = orc.Problem(n=(1, 1, 1), d=(1.0, 1.0, 1.0), periodic=(0, 0, 0), pbc_images=(0, 0, 0), materials=[m],
+                    g=fi.Globals(G11=1.0, G12=0.0, G44=0.5, G44p=0.5, eps0=1.0, epsB=1.0, L=1.0, E_ext=(0.0, 0.2, 0.0)))
+    o = orc.Oracle(p)
+    A, om, ph = np.array([0.0, 0.0, 0.8]), 3.0, 0.0
+    o.set_wave(A, om, ph)
+    P0 = np.array([0.0, 0.0, 0.3]).reshape(3, 1, 1, 1)
+    lam = 2.0 * 0.4
+
+    def exact_z(t):
+        return math.exp(-lam * t) * 0.3 + 0.8 * (lam * math.sin(om * t) - om * math.cos(om * t)
+                                                   + om * math.exp(-lam * t)) / (lam * lam + om * om)
+    return o, P0, exact_z
+
+
+@pytest.mark.parametrize("name,order", [("euler", 1), ("heun", 2), ("rk4", 4), ("ab3m2", 2), ("rk45", 5)])
+def test_time_dependent_field_is_sampled_at_the_stage_times(name, order):
+    """With a forcing that depends on t a wrong stage abscissa lowers the order of every multi-stage scheme."""
+    o, P0, exact_z = _forced_problem()
+    terms = orc.TERM_LANDAU | orc.TERM_EXT
+    T, errs = 2.3, []     # a time at which no leading error term vanishes by accident
+    for n in ((40, 80) if order < 5 else (12, 24)):
+        h = T / n
+        if name == "ab3m2":
+            P = o.step_ab3m2(P0, h, n, terms)
+        elif name == "rk45":
+            P = P0
+            for i in range(n):
+                P, st = o.step_rk45(P, h, h, 1e30, 4, terms, t0=i * h)
+        else:
+            P = o.step(P0, h, n, {"euler": orc.EULER, "heun": orc.HEUN, "rk4": orc.RK4}[name], terms)
+        errs.append(abs(P[2, 0, 0, 0] - exact_z(T)))
+        # the static y component relaxes to E_y / (2 a1_y) independently of the wave
+    ratio = errs[0] / errs[1]
+    assert 0.7 * 2 ** order < ratio < 1.45 * 2 ** order, (name, ratio)
+    # stepping in two calls with t0 equals one call
+    a = o.step(P0, 0.05, 10, orc.RK4, terms)
+    b = o.step(o.step(P0, 0.05, 4, orc.RK4, terms), 0.05, 6, orc.RK4, terms, t0=0.2)
+    assert np.allclose(a, b, rtol=0, atol=1e-15)
