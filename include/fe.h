@@ -92,6 +92,14 @@ fe_status fe_set_global(fe_grid* g, int32_t member, const fe_global* gl);
 fe_status fe_set_external_field(fe_grid* g, int32_t member, const double E[3]);
 /* dev_map: uint8 [nz][ny][nx] material id per cell, shared by the batch; NULL = all cells material 0.
  * Borrowed (not copied). */
+/* Time-dependent external excitation: E_ext(t) = E (fe_set_external_field) + amp sin(omega t + phase),
+ * sampled at the stage times of the integrator (t_n, t_n + dt/2, ... ; c_i h for RK45).  amp = 0 switches it off.
+ * The grid keeps a clock: fe_step / fe_step_rk45 advance it, fe_rhs and fe_energy sample E_ext at it. */
+fe_status fe_set_external_wave(fe_grid* g, int32_t member /* -1 = all */, const double amp[3], double omega,
+                               double phase);
+fe_status fe_set_time(fe_grid* g, double t);
+fe_status fe_get_time(const fe_grid* g, double* t);
+
 fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map);
 
 /* a0: cell-averaged dipolar tensor K_ij(d) on the padded box and its real spectrum (once per

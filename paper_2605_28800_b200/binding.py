@@ -23,7 +23,8 @@ FE_EULER, FE_HEUN, FE_RK4, FE_AB3M2 = 0, 1, 2, 3
 SYMBOLS = ["fe_create_grid", "fe_destroy_grid", "fe_workspace_bytes", "fe_bind_workspace", "fe_set_material",
            "fe_set_global", "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs",
            "fe_step", "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_launch_count", "fe_last_error",
-           "fe_version", "fe_profile", "fe_profile_read", "fe_step_rk45"]
+           "fe_version", "fe_profile", "fe_profile_read", "fe_step_rk45", "fe_set_external_wave", "fe_set_time",
+           "fe_get_time"]
 KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other"]
 
 
@@ -91,6 +92,9 @@ def load():
         L.fe_profile.argtypes = [vp, i32]
         L.fe_profile_read.argtypes = [vp, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_uint64), vp]
         L.fe_launch_count.argtypes = [vp]
+        L.fe_set_external_wave.argtypes = [vp, i32, ctypes.POINTER(dbl), dbl, dbl]
+        L.fe_set_time.argtypes = [vp, dbl]
+        L.fe_get_time.argtypes = [vp, ctypes.POINTER(dbl)]
         L.fe_step_rk45.argtypes = [vp, vp, dbl, dbl, dbl, i32, u32, ctypes.POINTER(fe_rk45_stats), vp]
         L.fe_launch_count.restype = ctypes.c_uint64
         L.fe_last_error.restype = ctypes.c_char_p
@@ -162,6 +166,21 @@ def fe_set_global(h, member: int, g):
 def fe_set_external_field(h, member: int, E):
     arr = (ctypes.c_double * 3)(*[float(v) for v in E])
     _check(load().fe_set_external_field(h, int(member), arr))
+
+
+def fe_set_external_wave(h, member: int, amp, omega: float, phase: float = 0.0):
+    a = (ctypes.c_double * 3)(*[float(v) for v in amp])
+    _check(load().fe_set_external_wave(h, int(member), a, float(omega), float(phase)))
+
+
+def fe_set_time(h, t: float):
+    _check(load().fe_set_time(h, float(t)))
+
+
+def fe_get_time(h) -> float:
+    t = ctypes.c_double(0.0)
+    _check(load().fe_get_time(h, ctypes.byref(t)))
+    return t.value
 
 
 def fe_set_material_map(h, dev_map: Optional[torch.Tensor]):
@@ -266,6 +285,9 @@ class Grid:
     def set_material(self, member, material_id, m): fe_set_material(self.h, member, material_id, m)
     def set_global(self, member, g): fe_set_global(self.h, member, g)
     def set_external_field(self, member, E): fe_set_external_field(self.h, member, E)
+    def set_external_wave(self, member, amp, omega, phase=0.0): fe_set_external_wave(self.h, member, amp, omega, phase)
+    def set_time(self, t): fe_set_time(self.h, t)
+    def time(self) -> float: return fe_get_time(self.h)
 
     def set_material_map(self, dev_map: Optional[torch.Tensor]):
         self._map = dev_map          # keep the borrowed tensor alive

@@ -71,6 +71,9 @@ struct fe_grid {
     cudaGraphExec_t gexec;
     bool gvalid, goff;               // cached graph usable / graphs disabled for this grid after a failure
     void* gP; double gdt; int ginteg; uint32_t gterms; uint64_t gunit_launches;
+    double time;                     // simulation time (advanced by fe_step / fe_step_rk45); E_ext(t) is sampled from it
+    double tstage;                   // time of the stage being evaluated
+    bool any_wave;                   // some member has a time-dependent excitation: no graph replay
     bool prof_on;
     std::vector<cudaEvent_t> prof_ev;
     std::vector<int> prof_kind;
@@ -239,6 +242,7 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     g->launches = 0;
     g->prof_on = false;
     g->prof_used = 0;
+    g->time = 0.0; g->tstage = 0.0; g->any_wave = false;
     g->gstream = nullptr; g->gev_in = nullptr; g->gev_out = nullptr; g->gexec = nullptr;
     g->gvalid = false; g->goff = false; g->gP = nullptr; g->gdt = 0.0; g->ginteg = -1; g->gterms = 0; g->gunit_launches = 0;
     const int B = d->batch, M = d->n_materials;
@@ -400,6 +404,39 @@ extern "C" fe_status fe_set_external_field(fe_grid* g, int32_t member, const dou
     return FE_OK;
 }
 
+extern "C" fe_status fe_set_external_wave(fe_grid* g, int32_t member, const double amp[3], double omega, double phase)
+{
+    if (!g || !amp) return fail(FE_EINVAL, "null argument");
+    const int B = g->desc.batch;
+    if (member < -1 || member >= B) return fail(FE_EINVAL, "member %d out of range", member);
+    if (!isfinite(amp[0]) || !isfinite(amp[1]) || !isfinite(amp[2]) || !isfinite(omega) || !isfinite(phase))
+        return fail(FE_EINVAL, "non-finite wave parameter");
+    const bool on = amp[0] != 0.0 || amp[1] != 0.0 || amp[2] != 0.0;
+    for (int b = (member < 0 ? 0 : member); b < (member < 0 ? B : member + 1); ++b) {
+        DevMember& dm = g->h_members[b];
+        for (int i = 0; i < 3; ++i) dm.wamp[i] = amp[i];
+        dm.womega = omega;
+        dm.wphase = phase;
+        dm.wave = on ? 1 : 0;
+    }
+    g->dirty = true;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_set_time(fe_grid* g, double t)
+{
+    if (!g || !isfinite(t)) return fail(FE_EINVAL, "bad argument");
+    g->time = t;
+    return FE_OK;
+}
+
+extern "C" fe_status fe_get_time(const fe_grid* g, double* t)
+{
+    if (!g || !t) return fail(FE_EINVAL, "null argument");
+    *t = g->time;
+    return FE_OK;
+}
+
 extern "C" fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map)
 {
     if (!g) return fail(FE_EINVAL, "null argument");
@@ -419,8 +456,11 @@ static fe_status sync_params(fe_grid* g, cudaStream_t st)
     if (!g->dirty) return FE_OK;
     g->gvalid = false;               // kernel variants (mixed term) may change with the coefficients
     g->mixed = 0;
-    for (int b = 0; b < B; ++b)
+    g->any_wave = false;
+    for (int b = 0; b < B; ++b) {
         if (g->h_members[b].Gm != 0.0) g->mixed = 1;
+        if (g->h_members[b].wave) g->any_wave = true;
+    }
     FE_CUDA(cudaMemcpyAsync(g->d_mats, g->h_mats.data(), (size_t)B * M * sizeof(DevLandau), cudaMemcpyHostToDevice, st));
     FE_CUDA(cudaMemcpyAsync(g->d_members, g->h_members.data(), (size_t)B * sizeof(DevMember), cudaMemcpyHostToDevice, st));
     // pageable host memory: the copies are staged before the calls return, the vectors may change afterwards
@@ -585,6 +625,7 @@ static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double c
     a.terms = terms;
     a.batch = g->desc.batch;
     a.mixed = g->mixed;
+    a.t = g->tstage;
     mark(g, K_LOCAL, st);
     FE_CUDA(launch_local<T>(a, st));
     g->launches += 1;
@@ -610,6 +651,7 @@ extern "C" fe_status fe_rhs(fe_grid* g, const void* P, void* dPdt, uint32_t term
     if (reinterpret_cast<uintptr_t>(dPdt) % 16) return fail(FE_EINVAL, "state arrays must be 16-byte aligned");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = sync_params(g, st)) != FE_OK) return s;
+    g->tstage = g->time;
     s = g->f32 ? stage<float>(g, (const float*)P, nullptr, (float*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st)
                : stage<double>(g, (const double*)P, nullptr, (double*)dPdt, 1.0, nullptr, nullptr, 0.0, terms, st);
     mark(g, -1, st);
@@ -617,7 +659,7 @@ extern "C" fe_status fe_rhs(fe_grid* g, const void* P, void* dPdt, uint32_t term
 }
 
 template <typename T>
-static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint32_t terms, cudaStream_t st)
+static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint32_t terms, cudaStream_t st, double t0)
 {
     T* Y = reinterpret_cast<T*>(g->ws + g->o_Y);
     T* ACC = reinterpret_cast<T*>(g->ws + g->o_ACC);
@@ -628,6 +670,7 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
         T* cur = P;
         T* nxt = PP;
         for (int i = 0; i < nsteps; ++i) {
+            g->tstage = t0 + i * dt;
             if ((s = stage<T>(g, cur, cur, nxt, dt, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
             T* t = cur; cur = nxt; nxt = t;
         }
@@ -638,7 +681,10 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
     } else if (integ == FE_HEUN) {
         for (int i = 0; i < nsteps; ++i) {
             // k1 = f(P): Y = P + dt k1, ACC = P + dt/2 k1;  k2 = f(Y): P = ACC + dt/2 k2
+            const double tn = t0 + i * dt;
+            g->tstage = tn;
             if ((s = stage<T>(g, P, P, Y, dt, P, ACC, 0.5 * dt, terms, st)) != FE_OK) return s;
+            g->tstage = tn + dt;
             if ((s = stage<T>(g, Y, ACC, P, 0.5 * dt, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
         }
     } else if (integ == FE_AB3M2) {
@@ -649,6 +695,8 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
         T* FS = reinterpret_cast<T*>(g->ws + g->o_K[3]);
         const int64_t n = (int64_t)g->desc.batch * 3 * g->N;
         for (int i = 0; i < nsteps; ++i) {
+            const double tn = t0 + i * dt;
+            g->tstage = tn;
             if ((s = stage<T>(g, P, nullptr, F[0], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
             LinArgs a;
             memset(&a, 0, sizeof(a));
@@ -661,6 +709,7 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
                 a.k[2] = F[2]; a.c[2] = dt * 5.0 / 12.0;
                 FE_CUDA(launch_lincomb<T>(Y, P, a, 3, n, st));
             }
+            g->tstage = tn + dt;
             if ((s = stage<T>(g, Y, nullptr, FS, 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
             memset(&a, 0, sizeof(a));
             a.k[0] = F[0]; a.c[0] = 0.5 * dt;
@@ -672,9 +721,13 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
     } else {
         for (int i = 0; i < nsteps; ++i) {
             // classical RK4, weights 1/6 1/3 1/3 1/6, stage points P + dt/2 k1, P + dt/2 k2, P + dt k3
+            const double tn = t0 + i * dt;
+            g->tstage = tn;
             if ((s = stage<T>(g, P, P, Y, 0.5 * dt, P, ACC, dt / 6.0, terms, st)) != FE_OK) return s;
+            g->tstage = tn + dt / 2.0;
             if ((s = stage<T>(g, Y, P, PP, 0.5 * dt, ACC, ACC, dt / 3.0, terms, st)) != FE_OK) return s;
             if ((s = stage<T>(g, PP, P, Y, dt, ACC, ACC, dt / 3.0, terms, st)) != FE_OK) return s;
+            g->tstage = tn + dt;
             if ((s = stage<T>(g, Y, ACC, P, dt / 6.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
         }
     }
@@ -690,16 +743,19 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
     if (integ != FE_EULER && integ != FE_HEUN && integ != FE_RK4 && integ != FE_AB3M2) return fail(FE_EINVAL, "unknown integrator");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = sync_params(g, st)) != FE_OK) return s;
+    const double time0 = g->time;
     auto run = [&](int n, cudaStream_t on) {
-        return g->f32 ? step_T<float>(g, (float*)P, dt, n, integ, terms, on) : step_T<double>(g, (double*)P, dt, n, integ, terms, on);
+        return g->f32 ? step_T<float>(g, (float*)P, dt, n, integ, terms, on, time0)
+                      : step_T<double>(g, (double*)P, dt, n, integ, terms, on, time0);
     };
     // Long runs replay a CUDA graph of one unit of steps (2 Euler steps: the ping-pong returns to P; 1 Heun / RK4 step)
     // on an internal stream ordered with the caller's stream by events: small grids are launch bound otherwise.
     // The first unit always runs eagerly (one-time kernel attribute set-up must not happen inside a capture).
     const int unit = integ == FE_EULER ? 2 : 1;
     static const bool graphs_off = getenv("FE_B200_GRAPH") && getenv("FE_B200_GRAPH")[0] == '0';
-    if (g->prof_on || g->goff || graphs_off || nsteps < 6 * unit || integ == FE_AB3M2) {
-        s = run(nsteps, st);
+    if (g->prof_on || g->goff || graphs_off || nsteps < 6 * unit || integ == FE_AB3M2 || g->any_wave) {
+        s = run(nsteps, st);             // (a time-dependent E_ext changes the kernel arguments from step to step)
+        if (s == FE_OK) g->time = time0 + nsteps * dt;
         mark(g, -1, st);
         return s;
     }
@@ -745,6 +801,7 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
         g->gvalid = false;
     }
     s = left > 0 ? run(left, st) : FE_OK;
+    if (s == FE_OK) g->time = time0 + nsteps * dt;
     mark(g, -1, st);
     return s;
 }
@@ -760,6 +817,7 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
                                    {3.0 / 10.0, -9.0 / 10.0, 6.0 / 5.0, 0, 0},
                                    {-11.0 / 54.0, 5.0 / 2.0, -70.0 / 27.0, 35.0 / 27.0, 0},
                                    {1631.0 / 55296.0, 175.0 / 512.0, 575.0 / 13824.0, 44275.0 / 110592.0, 253.0 / 4096.0}};
+    static const double C[6] = {0.0, 1.0 / 5.0, 3.0 / 10.0, 3.0 / 5.0, 1.0, 7.0 / 8.0};
     static const double B5[6] = {37.0 / 378.0, 0.0, 250.0 / 621.0, 125.0 / 594.0, 0.0, 512.0 / 1771.0};
     static const double B4[6] = {2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0, 277.0 / 14336.0, 1.0 / 4.0};
     T* K[6];
@@ -768,6 +826,7 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
     T* Y5 = reinterpret_cast<T*>(g->ws + g->o_PP);
     const int64_t n = (int64_t)g->desc.batch * 3 * g->N;
     const size_t bytes = (size_t)n * sizeof(T);
+    const double time0 = g->time;
     double t = 0.0, dt = dt_init, err = 0.0, dt_last = 0.0;
     int acc = 0, rej = 0, evals = 0;
     fe_status s;
@@ -785,6 +844,7 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
                 g->launches += 1;
                 Yi = Y;
             }
+            g->tstage = time0 + t + C[i] * h;
             if ((s = stage<T>(g, Yi, nullptr, K[i], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
         }
         evals += 6;
@@ -808,6 +868,7 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
         }
     }
     FE_CUDA(cudaStreamSynchronize(st));
+    g->time = time0 + t;
     if (out) { out->t = t; out->dt_last = dt_last; out->dt_next = dt; out->err_last = err;
                out->accepted = acc; out->rejected = rej; out->rhs_evals = evals; }
     return FE_OK;
@@ -854,6 +915,7 @@ extern "C" fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double
     a.partials = reinterpret_cast<double*>(g->ws + g->o_part);
     a.out = g->d_eout;
     a.nblk = g->nblk;
+    a.t = g->time;
     FE_CUDA(g->f32 ? launch_energy<float>(a, st) : launch_energy<double>(a, st));
     g->launches += 2;
     const size_t nb = (size_t)g->desc.batch * 8;

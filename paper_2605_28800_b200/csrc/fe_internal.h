@@ -33,6 +33,9 @@ struct DevMember {
     double escale;           // 1 / (eps0 * epsB)   (Eq. 6 prefactor)
     double L;
     double Eext[3];
+    // time-dependent excitation: E_ext(t) = Eext + wamp sin(womega t + wphase) when wave != 0
+    double wamp[3], womega, wphase;
+    int32_t wave, pad;
 };
 
 struct DevLandau {
@@ -144,6 +147,7 @@ struct LocalArgs {
     uint32_t terms;
     int batch;
     int mixed;            // any member has Gm != 0
+    double t;             // time at which E_ext is sampled (stage time)
     // filled by launch_local
     double id2[3];        // 1 / D_a^2
     double i4[3];         // 1 / (4 D_x D_y), 1 / (4 D_x D_z), 1 / (4 D_y D_z)
@@ -163,6 +167,7 @@ struct EnergyArgs {
     double d[3];
     uint32_t terms;
     int batch;
+    double t;             // time at which E_ext is sampled
     double* partials;     // [B][nblk][8]
     double* out;          // [B][8] device
     int nblk;

@@ -203,7 +203,9 @@ __global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
     const T ix = (T)a.id2[0], iy = (T)a.id2[1], iz = (T)a.id2[2];
     const T qxy = Gm * (T)a.i4[0], qxz = Gm * (T)a.i4[1], qyz = Gm * (T)a.i4[2];
     const T cy = (T)a.cy, ca = (T)a.ca;
-    const T ex0 = (T)mem.Eext[0], ex1 = (T)mem.Eext[1], ex2 = (T)mem.Eext[2];
+    const double wv = mem.wave ? sin(mem.womega * a.t + mem.wphase) : 0.0;      // E_ext sampled at the stage time
+    const T ex0 = (T)(mem.Eext[0] + mem.wamp[0] * wv), ex1 = (T)(mem.Eext[1] + mem.wamp[1] * wv),
+            ex2 = (T)(mem.Eext[2] + mem.wamp[2] * wv);
     const T* Ee = (a.terms & 4u) && a.Eelec ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
     const T* base = a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
     const bool base_is_Y = a.baseY == a.Y;
@@ -474,7 +476,9 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
     const T ix = (T)a.id2[0], iy = (T)a.id2[1], iz = (T)a.id2[2];
     const T qxy = Gm * (T)a.i4[0], qxz = Gm * (T)a.i4[1], qyz = Gm * (T)a.i4[2];
     const T cy = (T)a.cy, ca = (T)a.ca;
-    const T ex0 = (T)mem.Eext[0], ex1 = (T)mem.Eext[1], ex2 = (T)mem.Eext[2];
+    const double wv = mem.wave ? sin(mem.womega * a.t + mem.wphase) : 0.0;      // E_ext sampled at the stage time
+    const T ex0 = (T)(mem.Eext[0] + mem.wamp[0] * wv), ex1 = (T)(mem.Eext[1] + mem.wamp[1] * wv),
+            ex2 = (T)(mem.Eext[2] + mem.wamp[2] * wv);
     const T* Ee = (a.terms & 4u) && a.Eelec ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
     const T* base = a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
     const bool base_is_Y = a.baseY == a.Y;
@@ -698,6 +702,8 @@ __global__ void __launch_bounds__(256) k_energy(EnergyArgs a)
     Grid<T, MAP> g{{P, P + N, P + 2 * N}, a.map, mats, nx, ny, nz};
     double acc[kEn] = {0, 0, 0, 0, 0, 0, 0, 0};
     const double Gt = mem.Gt, G11 = mem.G11, Gm = mem.Gm;
+    const double wv = mem.wave ? sin(mem.womega * a.t + mem.wphase) : 0.0;
+    const double eex[3] = {mem.Eext[0] + mem.wamp[0] * wv, mem.Eext[1] + mem.wamp[1] * wv, mem.Eext[2] + mem.wamp[2] * wv};
     for (int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; r < N; r += (int64_t)gridDim.x * blockDim.x) {
         const int x = (int)(r % nx), y = (int)((r / nx) % ny), z = (int)(r / ((int64_t)nx * ny));
         const int c0[3] = {x, y, z};
@@ -713,7 +719,7 @@ __global__ void __launch_bounds__(256) k_energy(EnergyArgs a)
                 const T* Ee = static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N;
                 acc[2] -= 0.5 * ((double)Ee[r] * p0[0] + (double)Ee[N + r] * p0[1] + (double)Ee[2 * N + r] * p0[2]);
             }
-            if (a.terms & 8u) acc[3] -= mem.Eext[0] * p0[0] + mem.Eext[1] * p0[1] + mem.Eext[2] * p0[2];
+            if (a.terms & 8u) acc[3] -= eex[0] * p0[0] + eex[1] * p0[1] + eex[2] * p0[2];
             acc[4] += p0[0]; acc[5] += p0[1]; acc[6] += p0[2]; acc[7] += 1.0;
         }
         if (a.terms & 2u) {

@@ -81,3 +81,62 @@ def test_rk45_on_the_fast_path_and_batch_lockstep(fe):
     with pytest.raises(fe.FeError):
         g.step_rk45(P, 0.02, -1.0, 1e-7)
     g.close()
+
+
+def test_time_dependent_field_all_integrators(fe):
+    """Sinusoidal excitation on top of the static field, different per member, clock starting at t = 0.37:
+    RHS, energy and every integrator against the oracle (which samples E_ext at the stage times)."""
+    w = workload_from_random(87, (8, 8, 4), (0, 1, 0), (0, 2, 0), batch=2)
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    waves = [((0.3, -0.2, 0.5), 7.0, 0.4), ((-0.1, 0.6, 0.2), 3.0, -1.1)]
+    oracles = []
+    for b, (amp, om, ph) in enumerate(waves):
+        g.set_external_wave(b, amp, om, ph)
+        o = orc.Oracle(oracle_problem(w, b), elec="direct")
+        o.set_wave(amp, om, ph)
+        oracles.append(o)
+    t0, dt = 0.37, 8e-3
+    g.set_time(t0)
+    P = g.state(w.P0)
+    got = g.rhs(P).cpu().numpy()
+    for b in range(2):
+        assert rel_l2(got[b], oracles[b].rhs(w.P0[b], fi.TERM_ALL, t0)) < 1e-12
+    assert rel_l2(g.rhs(P, fi.TERM_EXT).cpu().numpy()[1], oracles[1].rhs(w.P0[1], fi.TERM_EXT, t0)) < 1e-13
+    for integ, name in ((fi.EULER, "euler"), (fi.HEUN, "heun"), (fi.RK4, "rk4"), (fe.FE_AB3M2, "ab3m2")):
+        g.set_time(t0)
+        P = g.state(w.P0)
+        g.step(P, dt, 12, integ, fi.TERM_ALL)              # long enough for the graph path, which must stay off
+        assert g.time() == pytest.approx(t0 + 12 * dt, rel=1e-15)
+        for b in range(2):
+            o = oracles[b]
+            want = (o.step_ab3m2(w.P0[b], dt, 12, fi.TERM_ALL, t0=t0) if name == "ab3m2"
+                    else o.step(w.P0[b], dt, 12, integ, fi.TERM_ALL, t0=t0))
+            assert rel_l2(P.cpu().numpy()[b], want) < 1e-12, (name, b)
+    # two calls continue the clock
+    g.set_time(t0)
+    Pa = g.state(w.P0)
+    g.step(Pa, dt, 5, fi.RK4, fi.TERM_ALL)
+    g.step(Pa, dt, 7, fi.RK4, fi.TERM_ALL)
+    want = oracles[0].step(w.P0[0], dt, 12, fi.RK4, fi.TERM_ALL, t0=t0)
+    assert rel_l2(Pa.cpu().numpy()[0], want) < 1e-12
+    # adaptive RK45 with the wave: single member so that the decisions can be compared
+    w1 = workload_from_random(89, (8, 8, 4), (0, 1, 0), (0, 2, 0), batch=1)
+    g1 = fe.Grid.from_workload(w1)
+    g1.precompute_tensor()
+    g1.set_external_wave(0, *waves[0])
+    o1 = orc.Oracle(oracle_problem(w1, 0), elec="direct")
+    o1.set_wave(*waves[0])
+    g1.set_time(t0)
+    P1 = g1.state(w1.P0)
+    st = g1.step_rk45(P1, 0.3, 0.05, 1e-7, 1000, fi.TERM_ALL)
+    want, so = o1.step_rk45(w1.P0[0], 0.3, 0.05, 1e-7, 1000, fi.TERM_ALL, t0=t0)
+    assert (st["accepted"], st["rejected"]) == (so["accepted"], so["rejected"])
+    assert rel_l2(P1.cpu().numpy()[0], want) < 1e-10
+    assert g1.time() == pytest.approx(t0 + 0.3, rel=1e-14)
+    e = g1.energy(P1)[0]
+    o1.p.g.E_ext = tuple(o1.e_ext(t0 + 0.3))               # the oracle's energy takes the field of that instant
+    o1.wave = None
+    assert np.allclose(e[:5], o1.energy(want)[:5], rtol=1e-9, atol=1e-11)
+    g.close()
+    g1.close()
