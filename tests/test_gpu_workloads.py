@@ -1,0 +1,77 @@
+"""-m gpu runs of the two schedule-type workloads (configs 3 and 4) through paper_2605_28800_b200.workloads at reduced
+length: the drivers only sequence C-ABI calls, so the checks are (i) equality with the same schedule issued by hand
+and parity of one leg with the oracle, (ii) the qualitative observables the configs name (readings A12, A13)."""
+import numpy as np
+import pytest
+
+import fe_inputs as fi
+from oracle import fe_oracle as orc
+from gpu_util import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fe():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2605_28800_b200 as fe
+    fe.load()
+    return fe
+
+
+def test_config3_temperature_sweep_schedule(fe):
+    from paper_2605_28800_b200 import workloads as wl
+    w = fi.config3(n=16, batch=16)
+    u = fi.Units(alpha_ref=abs(fi.batio3(300.0).a1[0]), P0=0.26, G110=5.1e-10)
+    mat = lambda b, leg: u.landau(fi.batio3(fi.config3_leg_temperature(b, leg)))
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    log = wl.temperature_sweep(g, P, mat, n_legs=3, steps_per_leg=40, dt=w.dt)
+    assert len(log) == 3 and log[0]["phases"].shape == (16, 4)
+    assert np.all(log[-1]["phases"].sum(axis=1) == w.cells)
+    # the same schedule through the oracle for one member (coefficients change between legs, state carries over)
+    b = 5
+    Pref = w.P0[b].copy()
+    for leg in range(3):
+        p = orc.Problem(n=w.n, d=w.d, periodic=w.periodic, pbc_images=w.pbc_images, materials=[mat(b, leg)],
+                        g=w.globals_[b], matmap=None)
+        Pref = orc.Oracle(p, elec="fft").step(Pref, w.dt, 40, fi.EULER, fi.TERM_ALL)
+    assert rel_l2(P.cpu().numpy()[b], Pref) < 1e-10
+    assert log[-1]["mean_abs_P"][b] == pytest.approx(np.linalg.norm(Pref, axis=0).mean(), rel=1e-10)
+    g.close()
+
+
+def test_config4_field_sweep_loop(fe):
+    """Reduced bilayer (32x32x16, image sum R = 2): a triangular E_z sweep of +-4e8 V/m (the paper's range,
+    PAPER.md:191-197; above the ~1.6e8 V/m intrinsic coercive field of Table 1's PbTiO3) switches <Pz>, and the
+    loop is hysteretic: at E_z = 0 the branch coming from +E and the one coming from -E differ in sign."""
+    from paper_2605_28800_b200 import workloads as wl
+    import torch
+    w = fi.config4(nxy=32, nz=16, pbc_images=2)
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P0 = np.zeros_like(w.P0)
+    P0[0, 2, 8:] = 0.9                                      # start poled up in the PbTiO3 layers
+    P = g.state(P0)
+    pts = [fi._pto_units().field(fi.config4_field(k, npoints=40, amp=4e8)) for k in range(41)]
+    loop = wl.field_sweep(g, P, pts, steps_per_point=150, dt=w.dt)[:, 0]
+    assert np.isfinite(loop).all()
+    k_pos, k_zero_down, k_neg, k_end = 10, 20, 30, 40
+    assert loop[k_pos] > 0.5 and loop[k_neg] < -0.5          # saturated along the field at both extremes
+    assert loop[k_zero_down] > 0.2 and loop[k_end] < -0.2    # remanence: opposite signs at E_z = 0 on the two branches
+    # SrTiO3 layers stay paraelectric: polarised only by the field, far less than PbTiO3
+    Pz = P.cpu().numpy()[0, 2]
+    assert abs(Pz[:8].mean()) < 0.5 * abs(Pz[8:].mean())
+    # hand-issued schedule gives the same state
+    g2 = fe.Grid.from_workload(w)
+    g2.precompute_tensor()
+    P2 = g2.state(P0)
+    for ez in pts:
+        g2.set_external_field(0, (0.0, 0.0, ez))
+        g2.step(P2, w.dt, 150, fi.EULER, fi.TERM_ALL)
+    assert torch.equal(P, P2)
+    g.close()
+    g2.close()
