@@ -61,7 +61,8 @@ typedef struct {
     int32_t dtype;             /* FE_F64 or FE_F32: type of every state array and of the arithmetic */
     int32_t n_materials;       /* M in 1..255: rows of the per-member coefficient table             */
     int32_t zero_mode;         /* != 0: with exactly two periodic axes, fix each plane sum of the
-                                  kernel to the infinite-film value (reading A4)          */
+                                  kernel to the infinite-film value; with three periodic axes remove
+                                  the mean of the kernel (k = 0 mode := 0) (reading A4)    */
 } fe_grid_desc;
 
 /* Landau coefficients of one material (Eq. 3, Table 1). a1 per axis. */

@@ -426,6 +426,17 @@ int orc_tensor_table(const int* n, const double* d, const int* periodic, const i
             }
         }
     }
+    if (zero_mode && np == 3) {
+        /* fully periodic box (reading A4, last case): the k = 0 mode of every component is set to 0 by removing the
+         * mean of the image-summed table, i.e. a uniformly polarised periodic crystal feels no field
+         * (short-circuit electrical boundary conditions). */
+        for (int comp = 0; comp < 6; ++comp) {
+            long double sum = 0;
+            for (int64_t i = 0; i < TT; ++i) sum += out[(int64_t)comp * TT + i];
+            double mean = (double)(sum / TT);
+            for (int64_t i = 0; i < TT; ++i) out[(int64_t)comp * TT + i] -= mean;
+        }
+    }
     return 0;
 }
 

@@ -481,7 +481,7 @@ static fe_status precompute_T(fe_grid* g, cudaStream_t st)
     const int64_t p64 = q.pitch64;
     for (int c = 0; c < 6; ++c) {
         FE_CUDA(launch_tensor_box(q, box, c, 1, st));
-        FE_CUDA(launch_zero_mode(q, box, c, st));
+        FE_CUDA(launch_zero_mode(q, box, c, g->d_eout, st));
         FE_CUDA(launch_xfwd<double>(g->ctx64, box, Sbox, q.m[0], q.m[1], q.m[2], q.m[0], (int64_t)q.m[0] * q.m[1],
                                     p64, p64 * q.m[1], st));
         FE_CUDA(launch_axis<double>(g->ctx64, 1, -1, Sbox, Sbox, q.m[1], q.lanes64, q.pitch64, q.m[2], 1, p64,
@@ -523,7 +523,7 @@ extern "C" fe_status fe_get_tensor(fe_grid* g, double* host_out, void* stream)
     const int64_t total = (int64_t)q.m[0] * q.m[1] * q.m[2];
     for (int c = 0; c < 6; ++c) {
         FE_CUDA(launch_tensor_box(q, box, c, 1, st));
-        FE_CUDA(launch_zero_mode(q, box, c, st));
+        FE_CUDA(launch_zero_mode(q, box, c, g->d_eout, st));
         FE_CUDA(cudaMemcpyAsync(host_out + c * total, box, total * sizeof(double), cudaMemcpyDeviceToHost, st));
         FE_CUDA(cudaStreamSynchronize(st));
         g->launches += 2;

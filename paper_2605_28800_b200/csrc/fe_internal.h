@@ -126,7 +126,8 @@ cudaError_t tensor_init_tables();
 // real-space kernel of one component on the circular box [mz][my][mx] (fp64)
 cudaError_t launch_tensor_box(const Geometry& g, double* box6 /* [6][mz][my][mx] or one comp */,
                               int comp_first, int ncomp, cudaStream_t st);
-cudaError_t launch_zero_mode(const Geometry& g, double* box, int comp, cudaStream_t st);
+cudaError_t launch_zero_mode(const Geometry& g, double* box, int comp, double* scratch /* one device double */,
+                             cudaStream_t st);
 
 // ---- local terms (fe_local.cu) ----------------------------------------------------------------
 struct LocalArgs {

@@ -274,9 +274,38 @@ __global__ void k_zero_mode(double* __restrict__ box, ZmArgs a)
     }
 }
 
-cudaError_t launch_zero_mode(const Geometry& g, double* box, int comp, cudaStream_t st)
+// Fully periodic box (reading A4, last case): remove the mean of the image-summed table (k = 0 mode := 0).
+__global__ void k_box_sum(const double* __restrict__ box, int64_t total, double* __restrict__ sum)
+{
+    __shared__ double red[256];
+    double s = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) s += box[i];
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int h = blockDim.x / 2; h > 0; h >>= 1) {
+        if ((int)threadIdx.x < h) red[threadIdx.x] += red[threadIdx.x + h];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) atomicAdd(sum, red[0]);
+}
+__global__ void k_box_shift(double* __restrict__ box, int64_t total, const double* __restrict__ sum)
+{
+    const double mean = *sum / (double)total;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) box[i] -= mean;
+}
+
+cudaError_t launch_zero_mode(const Geometry& g, double* box, int comp, double* scratch, cudaStream_t st)
 {
     const int np = g.periodic[0] + g.periodic[1] + g.periodic[2];
+    if (g.zero_mode && np == 3) {
+        const int64_t total = (int64_t)g.m[0] * g.m[1] * g.m[2];
+        cudaError_t e = cudaMemsetAsync(scratch, 0, sizeof(double), st);
+        if (e != cudaSuccess) return e;
+        const int grid = (int)((total + 255) / 256 < 1184 ? (total + 255) / 256 : 1184);
+        k_box_sum<<<grid, 256, 0, st>>>(box, total, scratch);
+        k_box_shift<<<grid, 256, 0, st>>>(box, total, scratch);
+        return cudaGetLastError();
+    }
     if (!g.zero_mode || np != 2) return cudaSuccess;
     ZmArgs a;
     for (int i = 0; i < 3; ++i) { a.m[i] = g.m[i]; a.n[i] = g.n[i]; }

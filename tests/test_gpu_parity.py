@@ -53,6 +53,30 @@ def test_tensor_table_matches_the_float128_oracle(fe, n, d, periodic, images):
         assert np.max(np.abs(tr)) < 1e-13
 
 
+def test_fully_periodic_box(fe):
+    """Three periodic axes (reading A4, last case): tensor table with the mean removed, RHS against the direct sum,
+    no field in a uniformly polarised periodic crystal."""
+    n, d, per, img = (8, 4, 8), (1.0, 1.1, 0.9), (1, 1, 1), (2, 2, 2)
+    g = fe.Grid(n, d, per, img, 1, "f64", 1)
+    K = g.get_tensor()
+    p = orc.Problem(n=n, d=d, periodic=per, pbc_images=img, materials=[fi.batio3(300.0)], g=fi.Globals(**fi.BATIO3_G))
+    ref = orc.circular_kernel(p, orc.tensor_table(p))
+    assert np.max(np.abs(K - ref)) < 1e-13          # 125 images summed in fp64 on the GPU, __float128 in the oracle
+    assert np.max(np.abs(K.reshape(6, -1).sum(axis=1))) < 1e-12
+    w = workload_from_random(33, n, per, img, batch=1)
+    g = _grid(fe, w)
+    o = orc.Oracle(oracle_problem(w), elec="direct")
+    for terms in (fi.TERM_ELEC, fi.TERM_ALL):
+        assert rel_l2(g.rhs(g.state(w.P0), terms).cpu().numpy()[0], o.rhs(w.P0[0], terms)) < TOL_RHS64
+    w2 = fi.open_batio3("per3", (16, 16, 8), 1, "f64", 7)
+    w2.periodic, w2.pbc_images = (1, 1, 1), (1, 1, 1)
+    g2 = _grid(fe, w2)
+    Pu = np.zeros_like(w2.P0)
+    Pu[0, 0], Pu[0, 2] = 0.4, -0.3
+    E = g2.rhs(g2.state(Pu), fi.TERM_ELEC).cpu().numpy()
+    assert np.max(np.abs(E)) < 1e-11 * (0.4 / (w2.globals_[0].eps0 * w2.globals_[0].epsB))
+
+
 def test_far_field_quadrature_tiers_against_the_oracle(fe):
     """Offsets up to 255 cells along x exercise every quadrature tier (8/6/4/3/2 nodes)."""
     n, d = (256, 4, 4), (1.0, 1.0, 1.0)

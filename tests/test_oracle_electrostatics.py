@@ -138,3 +138,45 @@ def test_electrostatic_operator_is_symmetric_positive():
         E1, E2 = orc.field_direct(p, K, P1), orc.field_direct(p, K, P2)
         assert np.sum(E1 * P2) == pytest.approx(np.sum(E2 * P1), rel=1e-12)
         assert -0.5 * np.sum(E1 * P1) > 0
+
+
+def test_fully_periodic_box_zero_mode_and_plane_wave():
+    """Three periodic axes (reading A4, last case): the mean of the kernel is removed, so (i) a uniformly polarised
+    periodic crystal feels no field, (ii) the field of a longitudinal plane wave P = e_x cos(2 pi x / n) approaches the
+    continuum value -P / (eps0 epsB) (all of it is bound charge), a transverse one P = e_y cos(2 pi x / n) ~ 0, as
+    the image sum grows, and (iii) with zero_mode off the mean is left in (plain image sum, Lorentz-type value 1/3
+    per diagonal component for cubic cells)."""
+    n = (8, 8, 8)
+    p = _problem(n, periodic=(1, 1, 1), images=(3, 3, 3), eps0=0.5, epsB=2.0)
+    K = orc.tensor_table(p)
+    for comp in range(6):
+        assert abs(K[comp].sum()) < 1e-12
+    P = np.zeros(p.shape)
+    P[0], P[1], P[2] = 0.3, -0.2, 0.7
+    np.testing.assert_allclose(orc.field_direct(p, K, P), 0.0, atol=1e-12)
+    x = np.arange(8)
+    wave = np.cos(2 * np.pi * x / 8)[None, None, :]
+    P = np.zeros(p.shape)
+    P[0] += wave
+    E = orc.field_fft(p, K, P)
+    # longitudinal response of the cell-averaged, image-summed kernel at k = 2 pi / (8 cells): within 1 % of the continuum
+    nodes = np.abs(wave[0, 0]) < 0.1
+    ratio = E[0, 0, 0, ~nodes] / (-wave[0, 0, ~nodes] / (0.5 * 2.0))
+    assert np.allclose(ratio, ratio[0], rtol=1e-10) and 0.99 < ratio[0] < 1.0
+    assert np.max(np.abs(E[0, 0, 0, nodes])) < 1e-12
+    np.testing.assert_allclose(E[1:], 0.0, atol=1e-12)
+    P = np.zeros(p.shape)
+    P[1] += wave                                     # transverse: no bound charge
+    Et = orc.field_fft(p, K, P)
+    assert np.max(np.abs(Et)) < 0.05 * np.max(np.abs(E))
+    # FFT = direct sum on this geometry too
+    Pr = np.random.default_rng(2).standard_normal(p.shape)
+    Ed, Ef = orc.field_direct(p, K, Pr), orc.field_fft(p, K, Pr)
+    assert np.linalg.norm(Ef - Ed) / np.linalg.norm(Ed) < 1e-13
+    p0 = _problem(n, periodic=(1, 1, 1), images=(3, 3, 3), eps0=0.5, epsB=2.0)
+    p0.zero_mode = False
+    K0 = orc.tensor_table(p0)
+    for comp in range(3):                            # cubic symmetry: each diagonal sum = trace / 3, trace of the sum = 1
+        assert K0[comp].sum() == pytest.approx(1.0 / 3.0, abs=1e-12)
+    for comp in range(3, 6):
+        assert abs(K0[comp].sum()) < 1e-12
