@@ -301,6 +301,30 @@ def config4_field_reduced(k: int) -> float:
     return _pto_units().field(config4_field(k))
 
 
+def strain_bilayer(nxy: int = 16, n_pto: int = 8, n_sto: int = 2, margin: int = 2, cell_nm: float = 0.5,
+                   r_s: float = 1.0, seed: int = 1007) -> Workload:
+    """PbTiO3 on SrTiO3 island surrounded by vacuum (Sec. 4.4): open boundaries, material map with
+    ids 0 = PbTiO3 (alpha_1z scaled by the strain parameter r_s), 1 = SrTiO3, 2 = vacuum (margin cells on
+    every side), the paper's gradient coefficients for this study (G11 = 3.46e-10, G12 = 0, G44 = G44' = 1.73e-10),
+    0.5 nm cells, 300 K, epsB = 649, random initial polarisation in PbTiO3 for r_s = 1."""
+    u = _pto_units()
+    nx = ny = nxy + 2 * margin
+    nz = n_pto + n_sto + 2 * margin
+    matmap = np.full((nz, ny, nx), 2, dtype=np.uint8)
+    matmap[margin:margin + n_sto, margin:-margin, margin:-margin] = 1
+    matmap[margin + n_sto:margin + n_sto + n_pto, margin:-margin, margin:-margin] = 0
+    P = np.zeros((1, 3, nz, ny, nx))
+    rnd = sphere_uniform(np.random.default_rng(seed), (nz, ny, nx), 0.7584 / u.P0)
+    P[0] = rnd * (matmap == 0)[None]
+    g = u.globals(Globals(G11=3.46e-10, G12=0.0, G44=1.73e-10, G44p=1.73e-10, epsB=649.0))
+    h = u.length(cell_nm * 1e-9)
+    return Workload(name=f"strain_bilayer_{nx}x{ny}x{nz}_rs{r_s:g}", n=(nx, ny, nz), d=(h, h, h), periodic=(0, 0, 0),
+                    pbc_images=(0, 0, 0), batch=1, dtype="f64",
+                    materials=[[u.landau(pbtio3(300.0, r_s)), u.landau(srtio3(300.0)), VACUUM]], globals_=[g],
+                    matmap=matmap, P0=P, dt=0.005, integrator=EULER, nsteps=2000,
+                    notes="strain sweep: set material 0 to Units.landau(pbtio3(300, r_s)) per leg, state carries over")
+
+
 def landau_ensemble(temperatures: Sequence[float] = tuple(10.0 * j for j in range(37)),
                     n: Tuple[int, int, int] = (16, 16, 8), seed: int = 1006) -> Workload:
     """Landau-only ensemble (Fig. 2): one batch member per temperature

@@ -47,3 +47,18 @@ def field_sweep(g: Grid, P: torch.Tensor, fields_z: Sequence[float], steps_per_p
         g.step(P, dt, steps_per_point, FE_EULER, FE_TERM_ALL)
         loop[k] = g.energy(P)[:, 7]
     return loop
+
+
+def strain_sweep(g: Grid, P: torch.Tensor, materials: Sequence[object], steps_per_leg: int, dt: float,
+                 material_id: int = 0) -> np.ndarray:
+    """Strain study: leg l sets material `material_id` of every member to materials[l] (alpha_1z
+    scaled by r_s) and relaxes for steps_per_leg Euler steps from the previous leg's state (adiabatic continuation).
+    Returns per leg and member [<Px>, <Py>, <Pz>, <|Pz|> / <|P|>] over the cells of the whole grid."""
+    out = np.zeros((len(materials), g.batch, 4))
+    for leg, m in enumerate(materials):
+        g.set_material(-1, material_id, m)
+        g.step(P, dt, steps_per_leg, FE_EULER, FE_TERM_ALL)
+        out[leg, :, :3] = g.energy(P)[:, 5:8]
+        norm = torch.linalg.vector_norm(P, dim=1).mean(dim=(1, 2, 3))
+        out[leg, :, 3] = (P[:, 2].abs().mean(dim=(1, 2, 3)) / norm.clamp_min(1e-300)).cpu().numpy()
+    return out
