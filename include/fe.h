@@ -38,7 +38,7 @@ typedef struct fe_grid fe_grid;   /* opaque; created by fe_create_grid, freed by
 
 typedef enum {
     FE_OK = 0,
-    FE_EINVAL = 1,      /* bad argument (sizes not a power of two in 4..1024, batch < 1, dx <= 0, ...) */
+    FE_EINVAL = 1,      /* bad argument (unsupported sizes, batch < 1, dx <= 0, ...) */
     FE_ENOMEM = 2,      /* workspace too small / allocation of the small tables failed               */
     FE_ECUDA = 3,       /* a CUDA call failed; text in fe_last_error()                              */
     FE_ESTATE = 4,      /* call order: no workspace bound, tensor not precomputed, material unset    */
@@ -53,7 +53,8 @@ enum { FE_EULER = 0, FE_HEUN = 1, FE_RK4 = 2,     /* PAPER.md:117-119; RK4 = BAS
 
 /* Geometry of the batch (PAPER.md:113 uniform cells; PAPER.md:117 batch). */
 typedef struct {
-    int32_t nx, ny, nz;        /* cells per axis; each a power of two in [4, 1024]                  */
+    int32_t nx, ny, nz;        /* cells per axis.  Periodic axis: a power of two in [4, 1024].  Open axis:
+                                  2..512 cells (nx even), zero-padded to the next power of two >= 2 n */
     double  dx, dy, dz;        /* cell size > 0                                                     */
     int32_t periodic[3];       /* per axis: 0 = open (vacuum outside, FFT zero-padded to 2n), 1 = periodic */
     int32_t pbc_images[3];     /* R >= 0 image cells summed on each side of a periodic axis         */

@@ -177,7 +177,14 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     const int n[3] = {d->nx, d->ny, d->nz};
     const double dd[3] = {d->dx, d->dy, d->dz};
     for (int a = 0; a < 3; ++a) {
-        if (!pow2_in(n[a], 4, 1024)) return fail(FE_EINVAL, "n[%d] = %d is not a power of two in [4, 1024]", a, n[a]);
+        if (d->periodic[a] == 1) {
+            if (!pow2_in(n[a], 4, 1024))
+                return fail(FE_EINVAL, "n[%d] = %d: a periodic axis must be a power of two in [4, 1024]", a, n[a]);
+        } else {
+            // open axis: zero-padded to the next power of two >= 2 n, any length goes (x even: the R2C pass packs pairs)
+            if (n[a] < 2 || n[a] > 512) return fail(FE_EINVAL, "n[%d] = %d: an open axis must have 2..512 cells", a, n[a]);
+            if (a == 0 && (n[a] & 1)) return fail(FE_EINVAL, "n[0] = %d: an open x axis must have an even number of cells", n[a]);
+        }
         if (!(dd[a] > 0.0) || !isfinite(dd[a])) return fail(FE_EINVAL, "cell size d[%d] must be > 0", a);
         if (d->periodic[a] != 0 && d->periodic[a] != 1) return fail(FE_EINVAL, "periodic[%d] must be 0 or 1", a);
         if (d->pbc_images[a] < 0 || d->pbc_images[a] > 64) return fail(FE_EINVAL, "pbc_images[%d] out of range", a);
@@ -199,7 +206,8 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
         q.n[a] = n[a];
         q.periodic[a] = d->periodic[a];
         q.images[a] = d->periodic[a] ? d->pbc_images[a] : 0;
-        q.m[a] = d->periodic[a] ? n[a] : 2 * n[a];
+        q.m[a] = n[a];
+        if (!d->periodic[a]) { q.m[a] = 4; while (q.m[a] < 2 * n[a]) q.m[a] *= 2; }
         q.d[a] = dd[a];
     }
     q.zero_mode = d->zero_mode;

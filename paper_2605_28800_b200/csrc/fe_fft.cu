@@ -244,11 +244,10 @@ __global__ void __launch_bounds__(kThreads) k_xinv(const cx<T>* __restrict__ in,
             s[a.invperm[k] * kPitchX + r] = Z;
         }
     fft_tiles<T, +1>(s, kPitchX, 3, 1, 0, a.plan, tw);
-    const int nc = a.n_real >> 1;
-    const int lognc = 31 - __clz(nc);
+    const int nc = a.n_real >> 1;            // any value up to Mc (open axes need not be powers of two)
     T* ob = out + (int64_t)blockIdx.x * a.real_ss + (int64_t)row0 * a.real_rs;
-    for (int idx = threadIdx.x; idx < (kRowsX << lognc); idx += blockDim.x) {
-        const int r = idx >> lognc, j = idx & (nc - 1);
+    for (int idx = threadIdx.x; idx < kRowsX * nc; idx += blockDim.x) {
+        const int r = idx / nc, j = idx - r * nc;
         if (r < nrow) *reinterpret_cast<cx<T>*>(ob + r * a.real_rs + 2 * j) = s[j * kPitchX + r];
     }
 }

@@ -13,6 +13,7 @@ namespace v2 {
 // same kernels serve the row-major spectra and the tiled layouts of fe_api.cu.
 struct Axis2Args {
     const void* tw;
+    int n_keep;       // rows that carry data on the pruned side (<= M/2 on a zero-padded axis)
     int64_t in_sa, in_s0, in_s1, in_sb, out_sa, out_s0, out_s1, out_sb;
 };
 
@@ -37,7 +38,7 @@ k2_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis2Args a)
     static_for<NLOAD>([&](auto ic) {
         constexpr int n1 = decltype(ic)::value;
         const int row = tp + R2 * n1;
-        v[n1] = ib[(int64_t)row * a.in_sa];
+        v[n1] = (!PIN || row < a.n_keep) ? ib[(int64_t)row * a.in_sa] : cx<T>{0, 0};
     });
     load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, LANES * TPP);
     __syncthreads();
@@ -66,7 +67,7 @@ k2_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis2Args a)
             constexpr int k2 = brev<R2>(p);
             if constexpr (!POUT || k2 < R2 / 2) {
                 const int row = k1 + R1 * k2;
-                ob[(int64_t)row * a.out_sa] = u[p];
+                if (!POUT || row < a.n_keep) ob[(int64_t)row * a.out_sa] = u[p];
             }
         });
     }
@@ -109,7 +110,7 @@ k3_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis2Args a)
         const int j = tp + it * TPP;
         static_for<NLOAD>([&](auto ic) {
             constexpr int n1 = decltype(ic)::value;
-            va[it][n1] = ib[(int64_t)(j + RB * RC * n1) * a.in_sa];
+            va[it][n1] = (!PIN || j + RB * RC * n1 < a.n_keep) ? ib[(int64_t)(j + RB * RC * n1) * a.in_sa] : cx<T>{0, 0};
         });
     }
     load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, 256);
@@ -155,7 +156,9 @@ k3_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis2Args a)
         static_for<RC>([&](auto pc) {
             constexpr int p = decltype(pc)::value;
             constexpr int k3 = brev<RC>(p);
-            if constexpr (!POUT || k3 < RC / 2) ob[(int64_t)(tc + RA * RB * k3) * a.out_sa] = u[p];
+            if constexpr (!POUT || k3 < RC / 2) {
+                if (!POUT || tc + RA * RB * k3 < a.n_keep) ob[(int64_t)(tc + RA * RB * k3) * a.out_sa] = u[p];
+            }
         });
     }
 }
@@ -198,6 +201,7 @@ static cudaError_t launch_m3(int dir, bool prune, const void* in, void* out, con
 struct Axis4Args {
     const void* tw;
     int n0, n1, ntiles;                   // tile t -> (t % n0, (t / n0) % n1, t / (n0 n1))
+    int n_keep;                           // data rows on the pruned side (<= M/2)
     int64_t in_s0, in_s1, in_sb, out_s0, out_s1, out_sb;
 };
 
@@ -255,8 +259,8 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
     constexpr int NB = 3;
     constexpr int TILE = M * LANES;
     constexpr bool PIN = PRUNE && DIR < 0, POUT = PRUNE && DIR > 0;
-    constexpr unsigned in_bytes = (unsigned)((PIN ? M / 2 : M) * LANES * sizeof(cx<T>));
-    constexpr unsigned out_bytes = (unsigned)((POUT ? M / 2 : M) * LANES * sizeof(cx<T>));
+    const unsigned in_bytes = (unsigned)((PIN ? a.n_keep : M) * LANES * sizeof(cx<T>));
+    const unsigned out_bytes = (unsigned)((POUT ? a.n_keep : M) * LANES * sizeof(cx<T>));
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(fe2_smem);     // [NB], 64 bytes reserved
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem + 64);
     cx<T>* bufs = tw + M;
@@ -292,6 +296,11 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
         const int b = i % NB;
         cx<T>* buf = bufs + b * TILE + lane;
         mbar_wait(&bars[b], (unsigned)((i / NB) & 1));
+        if (PIN && a.n_keep < M / 2) {
+            // the zero padding below M/2 is not part of the tile in memory: clear the rows the previous tile left there
+            for (int e = a.n_keep * LANES + threadIdx.x; e < (M / 2) * LANES; e += THREADS) bufs[b * TILE + e] = cx<T>{0, 0};
+            __syncthreads();
+        }
         if (DIR < 0) {
             // ---- A: task j = n3 + RC n2, slots j + RB RC n1
 #pragma unroll
@@ -471,9 +480,9 @@ cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, voi
                          int64_t out_s0, int64_t out_s1, int64_t out_sb, cudaStream_t st)
 {
     const int M = c.plan[axis].M;
-    v2::Axis2Args a{c.tw, in_sa, in_s0, in_s1, in_sb, out_sa, out_s0, out_s1, out_sb};
+    v2::Axis2Args a{c.tw, n_keep, in_sa, in_s0, in_s1, in_sb, out_sa, out_s0, out_s1, out_sb};
     dim3 grid(n0, n1, batch);
-    const bool prune = 2 * n_keep == M;
+    const bool prune = 2 * n_keep <= M;          // zero-padded axis
     if (!prune && n_keep != M) return cudaErrorInvalidValue;
     static const bool three_level = getenv("FE_B200_Y3") && getenv("FE_B200_Y3")[0] == '1';   // tuning aid
     if (three_level) {
@@ -515,9 +524,9 @@ cudaError_t launch_axis4(const FftCtx& c, int axis, int dir, const void* in, voi
                          int64_t out_sb, cudaStream_t st)
 {
     const int M = c.plan[axis].M;
-    const bool prune = 2 * n_keep == M;
+    const bool prune = 2 * n_keep <= M;          // zero-padded axis
     if (!prune && n_keep != M) return cudaErrorInvalidValue;
-    v2::Axis4Args a{c.tw, n0, n1, n0 * n1 * batch, in_s0, in_s1, in_sb, out_s0, out_s1, out_sb};
+    v2::Axis4Args a{c.tw, n0, n1, n0 * n1 * batch, n_keep, in_s0, in_s1, in_sb, out_s0, out_s1, out_sb};
     static const bool t512 = getenv("FE_B200_Y4T") && atoi(getenv("FE_B200_Y4T")) == 512;   // tuning aid
     if (M == 256) return v2::launch_m4<T, 256, 256>(dir, prune, in, out, a, st);
     if (M == 512) return t512 ? v2::launch_m4<T, 512, 512>(dir, prune, in, out, a, st) : v2::launch_m4<T, 512, 256>(dir, prune, in, out, a, st);

@@ -19,6 +19,7 @@ struct X2Args {
     int64_t real_rs;
     int ny, lg;
     int64_t s_plane, s_row, s_g;
+    int nc;         // valid complex pairs (x[2j], x[2j+1]) per real row: n_x / 2 (<= M/2 on a zero-padded axis, M otherwise)
 };
 __device__ __forceinline__ int64_t spec_off(const X2Args& a, int k) { return (int64_t)(k >> a.lg) * a.s_g + (k & ((1 << a.lg) - 1)); }
 __device__ __forceinline__ int64_t spec_row(const X2Args& a, int64_t row) { return (row / a.ny) * a.s_plane + (row % a.ny) * a.s_row; }
@@ -48,7 +49,10 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
     constexpr int NLOAD = PRUNE ? R1 / 2 : R1;
     if (live) {
         const cx<T>* src = reinterpret_cast<const cx<T>*>(in + row * a.real_rs) + tp;
-        static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = src[R2 * decltype(ic)::value]; });
+        static_for<NLOAD>([&](auto ic) {
+            constexpr int n1 = decltype(ic)::value;
+            v[n1] = (!PRUNE || tp + R2 * n1 < a.nc) ? src[R2 * n1] : cx<T>{0, 0};
+        });
     } else {
         static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = cx<T>{0, 0}; });
     }
@@ -156,7 +160,9 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
             static_for<R2>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
                 constexpr int o2 = brev<R2>(p);
-                if constexpr (!PRUNE || o2 < R2 / 2) dst[R1 * o2] = u[p];
+                if constexpr (!PRUNE || o2 < R2 / 2) {
+                    if (!PRUNE || o1 + R1 * o2 < a.nc) dst[R1 * o2] = u[p];
+                }
             });
         }
     }
@@ -210,11 +216,11 @@ cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, in
                          const int64_t spec[4], int lanes, cudaStream_t st)
 {
     const int M = c.plan[0].M;
-    const bool prune = n_real == M;
-    if (!prune && n_real != 2 * M) return cudaErrorInvalidValue;
+    const bool prune = n_real <= M;          // zero-padded axis: at most half of the 2 M reals are data
+    if ((!prune && n_real != 2 * M) || (n_real & 1)) return cudaErrorInvalidValue;
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
-    v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3]};
+    v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2};
     return v2::launch_x<T, true>(M, prune, in, out, a, st);
 }
 
@@ -223,11 +229,11 @@ cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, in
                          const int64_t spec[4], int lanes, cudaStream_t st)
 {
     const int M = c.plan[0].M;
-    const bool prune = n_real == M;
-    if (!prune && n_real != 2 * M) return cudaErrorInvalidValue;
+    const bool prune = n_real <= M;          // zero-padded axis: at most half of the 2 M reals are data
+    if ((!prune && n_real != 2 * M) || (n_real & 1)) return cudaErrorInvalidValue;
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
-    v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3]};
+    v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2};
     return v2::launch_x<T, false>(M, prune, in, out, a, st);
 }
 

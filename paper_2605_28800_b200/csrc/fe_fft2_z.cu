@@ -30,7 +30,7 @@ template <> struct ZFact<256> { static constexpr int R1 = 32, R2 = 8; };
 struct Z2Args {
     const void* tw;
     const DevMember* members;
-    int My, batch;
+    int My, batch, nz;         // nz: data rows per pencil (<= M/2 on a zero-padded axis)
     int ngroups;      // groups of LANES consecutive kx
     int nitems;       // ngroups * (My/2 + 1)
     int64_t cs, s_z, s_ky, s_g;
@@ -139,7 +139,8 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         for (int c = 0; c < 3; ++c) {
 #pragma unroll
             for (int j = 0; j < NIN / RSTEP; ++j)
-                cp_async_n<CB>(s + (c * NIN + j * RSTEP) * LANES, g + c * cs + (int64_t)(j * RSTEP) * sa);
+                if (!PRUNE || row0 + j * RSTEP < a.nz)          // rows nz .. M/2 of a zero-padded axis stay zero
+                    cp_async_n<CB>(s + (c * NIN + j * RSTEP) * LANES, g + c * cs + (int64_t)(j * RSTEP) * sa);
         }
     };
     auto prefetch_k = [&](const ZIter& it) {
@@ -164,6 +165,10 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     ZIter cur;
     cur.set_item(blockIdx.x, a);
     if (!cur.valid(a)) return;
+    if (PRUNE && a.nz < NIN) {              // padding rows inside the staged half: cleared once, never written again
+        for (int e = threadIdx.x; e < 3 * NIN * LANES; e += C::THREADS) stage[e] = cx<T>{0, 0};
+        __syncthreads();
+    }
     prefetch_tile(cur);
     cp_async_commit();                      // group A: input of the first tile
     prefetch_k(cur);
@@ -262,7 +267,9 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                 static_for<R1>([&](auto pc) {
                     constexpr int p = decltype(pc)::value;
                     constexpr int n1 = brev<R1>(p);
-                    if constexpr (!PRUNE || n1 < R1 / 2) out[(int64_t)(R2 * n1) * sa] = w[p];
+                    if constexpr (!PRUNE || n1 < R1 / 2) {
+                        if (!PRUNE || R2 * n1 + n2 < a.nz) out[(int64_t)(R2 * n1) * sa] = w[p];
+                    }
                 });
             }
         }
@@ -311,9 +318,9 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
 {
     const int M = c.plan[2].M;
     constexpr int L128 = 128 / (int)sizeof(v2::cx<T>);      // lanes of a 128-byte row
-    v2::Z2Args a{c.tw, members, My, batch, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
+    v2::Z2Args a{c.tw, members, My, batch, nz, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
                  kstr[0], kstr[1], kstr[2], kstr[3], perm[0], perm[1], perm[2]};
-    const bool prune = 2 * nz == M;
+    const bool prune = 2 * nz <= M;              // zero-padded axis
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
         case 64: return v2::launch_p<T, 64, L128>(prune, S, Kt, a, st);

@@ -184,8 +184,8 @@ struct BoxArgs {
     int comp_first, ncomp;
 };
 
-// One thread per box entry.  Open axis: index t holds offset t (t < n), t - m (t > n), and 0 at t = n
-// (never a pair offset).  Periodic axis: minimum image of t, the tie |d| = n/2 is the mean of both signs;
+// One thread per box entry.  Open axis (m >= 2 n): index t holds offset t (t < n), t - m (t > m - n), and 0 for
+// n <= t <= m - n (never a pair offset).  Periodic axis: minimum image of t, the tie |d| = n/2 is the mean of both signs;
 // K = sum over images q in [-R, R] of N(d + q n) (reading A4).
 __global__ void k_tensor_box(double* __restrict__ box, BoxArgs a)
 {
@@ -200,7 +200,7 @@ __global__ void k_tensor_box(double* __restrict__ box, BoxArgs a)
         if (!a.periodic[ax]) {
             cnt[ax] = 1;
             if (t[ax] < n) lo[ax] = t[ax];
-            else if (t[ax] == n) { lo[ax] = 0; unused = true; }
+            else if (t[ax] <= a.m[ax] - n) { lo[ax] = 0; unused = true; }      // n .. m - n: never a pair offset
             else lo[ax] = t[ax] - a.m[ax];
         } else {
             if (2 * t[ax] < n) { lo[ax] = t[ax]; cnt[ax] = 1; }
@@ -251,7 +251,7 @@ __global__ void k_zero_mode(double* __restrict__ box, ZmArgs a)
 {
     __shared__ double red[256];
     const int tw = blockIdx.x;
-    if (tw == a.n[a.w]) return;
+    if (tw >= a.n[a.w] && tw <= a.m[a.w] - a.n[a.w]) return;      // unused planes of the padded open axis
     const int u = (a.w + 1) % 3, v = (a.w + 2) % 3;
     const int64_t stride[3] = {1, a.m[0], (int64_t)a.m[0] * a.m[1]};
     const int cnt = a.m[u] * a.m[v];

@@ -55,7 +55,8 @@ def test_version_and_error_strings_without_gpu(lib):
     # argument validation happens before any CUDA call
     from paper_2605_28800_b200 import binding
     d = binding.fe_grid_desc()
-    d.nx, d.ny, d.nz = 12, 16, 8          # 12 is not a power of two
+    d.nx, d.ny, d.nz = 12, 16, 8          # 12 is not a power of two: refused on a periodic axis
+    d.periodic[0] = 1
     d.dx = d.dy = d.dz = 1.0
     d.batch, d.n_materials = 1, 1
     h = ctypes.c_void_p()

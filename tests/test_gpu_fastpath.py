@@ -182,6 +182,9 @@ def test_full_size_point_sources_against_closed_form(fe, cfg, dtype, tol):
     ((64, 128, 64), (0, 0, 0), (0, 0, 0), "f32"),        # bulk-copy y pass (256) in fp32
     ((256, 128, 16), (1, 1, 0), (1, 1, 0), "f64"),       # unpruned x, y; generic z
     ((16, 16, 8), (0, 0, 0), (0, 0, 0), "f64"),          # generic passes only
+    ((72, 40, 36), (0, 0, 0), (0, 0, 0), "f64"),         # open axes that are not powers of two (partial pruning)
+    ((36, 140, 70), (0, 0, 0), (0, 0, 0), "f32"),
+    ((12, 10, 6), (0, 0, 0), (0, 0, 0), "f64"),
 ])
 def test_no_write_outside_the_caller_buffers(fe, n, periodic, images, dtype):
     """Guard bands around the workspace, the state and the output (compute-sanitizer is closed on the pool): every byte
@@ -215,3 +218,40 @@ def test_no_write_outside_the_caller_buffers(fe, n, periodic, images, dtype):
         assert bool((buf[:pad] == 7.0).all()) and bool((buf[pad + numel:] == 7.0).all())
     assert bool(torch.isfinite(P).all()) and bool(torch.isfinite(O).all())
     g.close()
+
+
+@pytest.mark.parametrize("n,periodic,images", [
+    ((12, 10, 6), (0, 0, 0), (0, 0, 0)),          # generic passes, padded 32 x 32 x 16
+    ((72, 40, 36), (0, 0, 0), (0, 0, 0)),         # fast passes with partial pruning: Mc = 128, My = 128, Mz = 128
+    ((36, 140, 70), (0, 0, 0), (0, 0, 0)),        # Mc = 64, bulk-copy y pass (512, 140 data rows), Mz = 256 (70 data rows)
+    ((64, 36, 24), (1, 0, 0), (1, 0, 0)),         # periodic power-of-two x, open y and z of arbitrary length
+    ((100, 64, 12), (0, 1, 0), (0, 1, 0)),        # Mc = 128 (100 reals per row), periodic y, generic z
+])
+def test_open_axes_of_arbitrary_length(fe, n, periodic, images):
+    """Open axes need not be powers of two (the paper's own grids are 128 x 128 x 36, 80 x 80 x 80 ...): they are
+    zero-padded to the next power of two >= 2 n and the pruned passes skip the padding.  RHS against oracle-FFT (which
+    pads to 2 n exactly) and against the direct sum at sampled cells; a few Euler steps; guard bands."""
+    w = _workload(n, periodic, images)
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    o = orc.Oracle(oracle_problem(w), elec="fft")
+    P = g.state(w.P0)
+    for terms in (fi.TERM_ELEC, fi.TERM_ALL):
+        assert rel_l2(g.rhs(P, terms).cpu().numpy()[0], o.rhs(w.P0[0], terms)) < TOL_RHS64, terms
+    t = np.random.default_rng(4).integers(0, w.cells, size=5)
+    Ed = orc.field_direct(o.p, o.table(), w.P0[0], targets=t)
+    got_e = g.rhs(P, fi.TERM_ELEC).cpu().numpy()[0].reshape(3, -1)[:, t] / w.globals_[0].L
+    assert np.max(np.abs(got_e - Ed)) < 1e-10 * np.max(np.abs(Ed))
+    g.step(P, w.dt, 8, fi.EULER, fi.TERM_ALL)
+    assert rel_l2(P.cpu().numpy()[0], o.step(w.P0[0], w.dt, 8, fi.EULER, fi.TERM_ALL)) < 1e-11
+    e, eo = g.energy(P)[0], o.energy(o.step(w.P0[0], w.dt, 8, fi.EULER, fi.TERM_ALL))
+    assert np.allclose(e[:5], eo[:5], rtol=1e-9, atol=1e-10 * abs(eo[4]))
+    g.close()
+
+
+def test_odd_open_x_axis_is_refused(fe):
+    with pytest.raises(fe.FeError) as ei:
+        fe.Grid((13, 8, 8), (1.0, 1.0, 1.0))
+    assert ei.value.status == fe.FE_EINVAL
+    with pytest.raises(fe.FeError):
+        fe.Grid((12, 8, 8), (1.0, 1.0, 1.0), periodic=(1, 0, 0))      # periodic axes stay powers of two
