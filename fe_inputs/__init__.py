@@ -287,6 +287,26 @@ def config4(nxy: int = 128, nz: int = 32, pbc_images: int = 10, skyrmion: bool =
                     notes="field sweep: config4_field(k)")
 
 
+def config4_paper(nxy: int = 128, seed: int = 1004) -> Workload:
+    """The paper's own bilayer geometry: 128 x 128 x 36 cells of 1 nm, from the bottom 12 nm SrTiO3
+    (material 1), 20 nm PbTiO3 (material 0), 4 nm vacuum (material 2), open boundaries on all axes ("finite samples
+    embedded in vacuum", PAPER.md:76), epsB = 649.  BASELINE.json's config 4 is the periodic 128 x 128 x 32 variant."""
+    u = _pto_units()
+    Ps = 0.7584 / u.P0
+    nz = 36
+    matmap = np.full((nz, nxy, nxy), 2, dtype=np.uint8)
+    matmap[:12] = 1
+    matmap[12:32] = 0
+    P = np.zeros((1, 3, nz, nxy, nxy))
+    P[0, :, 12:32] = sphere_uniform(np.random.default_rng(seed), (20, nxy, nxy), Ps)
+    g = u.globals(Globals(**PBTIO3_G, epsB=649.0))
+    h = u.length(1e-9)
+    return Workload(name=f"cfg4_paper_{nxy}x{nxy}x{nz}", n=(nxy, nxy, nz), d=(h, h, h), periodic=(0, 0, 0),
+                    pbc_images=(0, 0, 0), batch=1, dtype="f64",
+                    materials=[[u.landau(pbtio3(300.0)), u.landau(srtio3(300.0)), VACUUM]], globals_=[g],
+                    matmap=matmap, P0=P, dt=0.02, integrator=EULER, nsteps=500)
+
+
 def config4_field(k: int, npoints: int = 200, amp: float = 1e8) -> float:
     """Triangular sweep 0 -> +amp -> -amp -> 0 over npoints (SI V/m)."""
     q = npoints // 4

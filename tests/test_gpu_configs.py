@@ -127,3 +127,23 @@ def test_config4_full_size_bilayer(fe, skyrmion):
     gl = w.globals_[0]
     assert np.allclose(Ez[2][p.active > 0], -gl.L * 0.3 / (gl.eps0 * gl.epsB), rtol=1e-11)
     g.close()
+
+
+def test_paper_bilayer_geometry_128x128x36(fe):
+    """The geometry the paper itself simulates: 128 x 128 x 36, SrTiO3 / PbTiO3 / vacuum layers, open on
+    every axis; z = 36 is not a power of two (transform length 128, 36 data rows)."""
+    w = fi.config4_paper()
+    assert w.n == (128, 128, 36)
+    p = oracle_problem(w)
+    o = orc.Oracle(p, elec="fft")
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    g.set_external_field(0, (0.0, 0.0, fi.config4_field_reduced(12)))
+    o.p.g.E_ext = (0.0, 0.0, fi.config4_field_reduced(12))
+    P = g.state(w.P0)
+    got = g.rhs(P).cpu().numpy()[0]
+    assert rel_l2(got, o.rhs(w.P0[0])) < 1e-10
+    assert np.all(got[:, w.matmap == 2] == 0.0)                   # vacuum layer
+    g.step(P, w.dt, 3, fi.EULER, fi.TERM_ALL)
+    assert rel_l2(P.cpu().numpy()[0], o.step(w.P0[0], w.dt, 3, fi.EULER, fi.TERM_ALL)) < 1e-10
+    g.close()
