@@ -21,29 +21,29 @@ namespace v2 {
 
 template <typename T> struct alignas(2 * sizeof(T)) cx { T x, y; };
 
-template <typename T> __device__ __forceinline__ cx<T> cadd(cx<T> a, cx<T> b) { return {a.x + b.x, a.y + b.y}; }
-template <typename T> __device__ __forceinline__ cx<T> csub(cx<T> a, cx<T> b) { return {a.x - b.x, a.y - b.y}; }
-template <typename T> __device__ __forceinline__ cx<T> cmul(cx<T> a, cx<T> b)
+template <typename T> __host__ __device__ __forceinline__ cx<T> cadd(cx<T> a, cx<T> b) { return {a.x + b.x, a.y + b.y}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> csub(cx<T> a, cx<T> b) { return {a.x - b.x, a.y - b.y}; }
+template <typename T> __host__ __device__ __forceinline__ cx<T> cmul(cx<T> a, cx<T> b)
 {
     return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x};
 }
-template <typename T> __device__ __forceinline__ cx<T> cmulc(cx<T> a, cx<T> b)   // a * conj(b)
+template <typename T> __host__ __device__ __forceinline__ cx<T> cmulc(cx<T> a, cx<T> b)   // a * conj(b)
 {
     return {a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y};
 }
 // a * w (DIR < 0) or a * conj(w) (DIR > 0), w from the forward-sign table
-template <typename T, int DIR> __device__ __forceinline__ cx<T> cmuld(cx<T> a, cx<T> w)
+template <typename T, int DIR> __host__ __device__ __forceinline__ cx<T> cmuld(cx<T> a, cx<T> w)
 {
     return DIR < 0 ? cmul(a, w) : cmulc(a, w);
 }
 
 template <int... I, typename F>
-__device__ __forceinline__ void static_for_impl(F&& f, std::integer_sequence<int, I...>)
+__host__ __device__ __forceinline__ void static_for_impl(F&& f, std::integer_sequence<int, I...>)
 {
     (f(std::integral_constant<int, I>{}), ...);
 }
 // f(integral_constant<int, 0>) ... f(integral_constant<int, N-1>): every index is a compile-time constant
-template <int N, typename F> __device__ __forceinline__ void static_for(F&& f)
+template <int N, typename F> __host__ __device__ __forceinline__ void static_for(F&& f)
 {
     static_for_impl(f, std::make_integer_sequence<int, N>{});
 }
@@ -77,7 +77,7 @@ __host__ __device__ constexpr double cos16(int i)
 __host__ __device__ constexpr double sin16(int i) { return cos16(8 - i); }
 
 // a * exp(DIR * 2 pi i * IDX / 32), 0 <= IDX < 16
-template <typename T, int DIR, int IDX> __device__ __forceinline__ cx<T> mulw32(cx<T> a)
+template <typename T, int DIR, int IDX> __host__ __device__ __forceinline__ cx<T> mulw32(cx<T> a)
 {
     constexpr T s = (T)DIR;
     if constexpr (IDX == 0) {
@@ -100,7 +100,7 @@ template <typename T, int DIR, int IDX> __device__ __forceinline__ cx<T> mulw32(
 // in-register decimation in frequency on v[OFF .. OFF+LEN): natural order in, v[OFF + p] = X[brev<LEN>(p)] out.
 // PRUNE: the upper half of the input is zero (first stage needs no additions).
 template <typename T, int DIR, int LEN, int OFF = 0, bool PRUNE = false> struct Dif {
-    static __device__ __forceinline__ void run(cx<T>* v)
+    static __host__ __device__ __forceinline__ void run(cx<T>* v)
     {
         constexpr int H = LEN / 2;
         static_for<H>([&](auto ic) {
@@ -121,12 +121,12 @@ template <typename T, int DIR, int LEN, int OFF = 0, bool PRUNE = false> struct 
     }
 };
 template <typename T, int DIR, int OFF, bool PRUNE> struct Dif<T, DIR, 1, OFF, PRUNE> {
-    static __device__ __forceinline__ void run(cx<T>*) {}
+    static __host__ __device__ __forceinline__ void run(cx<T>*) {}
 };
 
 // in-register decimation in time: v[OFF + p] = X[brev<LEN>(p)] in, natural order out
 template <typename T, int DIR, int LEN, int OFF = 0> struct Dit {
-    static __device__ __forceinline__ void run(cx<T>* v)
+    static __host__ __device__ __forceinline__ void run(cx<T>* v)
     {
         constexpr int H = LEN / 2;
         if constexpr (LEN > 2) {
@@ -143,7 +143,69 @@ template <typename T, int DIR, int LEN, int OFF = 0> struct Dit {
     }
 };
 template <typename T, int DIR, int OFF> struct Dit<T, DIR, 1, OFF> {
-    static __device__ __forceinline__ void run(cx<T>*) {}
+    static __host__ __device__ __forceinline__ void run(cx<T>*) {}
+};
+
+// ---- fused multiply-add butterflies (decimation in time) ----------------------------------------------------
+// a' = a + w b, b' = a - w b with w = exp(DIR * 2 pi i * IDX / 32), 0 <= IDX < 16.  For a general w = c + i s the
+// product is folded into the additions: with t = s / c (|c| >= |s|), b~ = (b.x - t b.y, b.y + t b.x) and
+// a +- w b = a +- c b~, six fused multiply-adds instead of the four multiplies and four additions of the plain
+// form; when |s| > |c| the roles of c and s are exchanged (w b = s (u b.x - b.y, u b.y + b.x), u = c / s) so that
+// the ratio never exceeds one.  HI = false drops b' (pruned output).
+__host__ __device__ __forceinline__ constexpr double cabs_c(double v) { return v < 0 ? -v : v; }
+template <typename T, int DIR, int IDX, bool HI = true>
+__host__ __device__ __forceinline__ void bfly_dit(cx<T>& a, cx<T>& b)
+{
+    if constexpr (IDX == 0) {
+        const cx<T> t = b;
+        if constexpr (HI) b = csub(a, t);
+        a = cadd(a, t);
+    } else if constexpr (IDX == 8) {                         // w = DIR * i
+        const cx<T> t = DIR > 0 ? cx<T>{-b.y, b.x} : cx<T>{b.y, -b.x};
+        if constexpr (HI) b = csub(a, t);
+        a = cadd(a, t);
+    } else {
+        constexpr double c = IDX <= 8 ? cos16(IDX) : -cos16(16 - IDX);
+        constexpr double s = (double)DIR * (IDX <= 8 ? sin16(IDX) : sin16(16 - IDX));
+        T br, bi, m;
+        if constexpr (cabs_c(c) >= cabs_c(s)) {
+            constexpr T t = (T)(s / c);
+            br = fma(-t, b.y, b.x);
+            bi = fma(t, b.x, b.y);
+            m = (T)c;
+        } else {
+            constexpr T u = (T)(c / s);
+            br = fma(u, b.x, -b.y);
+            bi = fma(u, b.y, b.x);
+            m = (T)s;
+        }
+        if constexpr (HI) b = {fma(-m, br, a.x), fma(-m, bi, a.y)};
+        a = {fma(m, br, a.x), fma(m, bi, a.y)};
+    }
+}
+
+// in-register decimation in time with the fused butterflies: v[OFF + p] = x[brev<LEN>(p)] in, v[OFF + k] = X[k] out.
+// PIN: x[n] = 0 for n >= LEN/2 (the odd positions p are never read); POUT: only X[k], k < LEN/2, are produced.
+template <typename T, int DIR, int LEN, int OFF = 0, bool PIN = false, bool POUT = false> struct DitF {
+    static __host__ __device__ __forceinline__ void run(cx<T>* v)
+    {
+        constexpr int H = LEN / 2;
+        if constexpr (LEN == 2 && PIN) {
+            v[OFF + 1] = v[OFF];
+        } else {
+            if constexpr (LEN > 2) {
+                DitF<T, DIR, H, OFF, PIN, false>::run(v);
+                DitF<T, DIR, H, OFF + H, PIN, false>::run(v);
+            }
+            static_for<H>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                bfly_dit<T, DIR, i * (32 / LEN), !POUT>(v[OFF + i], v[OFF + i + H]);
+            });
+        }
+    }
+};
+template <typename T, int DIR, int OFF, bool PIN, bool POUT> struct DitF<T, DIR, 1, OFF, PIN, POUT> {
+    static __host__ __device__ __forceinline__ void run(cx<T>*) {}
 };
 
 // factorisation M = R1 * R2 (R1 >= R2) of the supported lengths

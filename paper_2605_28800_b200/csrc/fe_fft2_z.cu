@@ -10,8 +10,10 @@
 //                previous tile is being transformed.
 // Per tile, one thread holds the spectrum of all three components at the R2 frequencies kz = k1 + R1 k2 in
 // registers, so the multiply and the first stage of the inverse transform need no shared-memory round trip:
-//   forward   x[n2 + R2 n1] -> (R1-point over n1) -> twiddle -> exchange -> (R2-point over n2) -> X[k1 + R1 k2]
+//   forward   x[n2 + R2 n1] -> (R1-point over n1) -> exchange -> twiddle -> (R2-point over n2) -> X[k1 + R1 k2]
 //   inverse   X[k1 + R1 k2] -> (R2-point over k2) -> twiddle -> exchange -> (R1-point over k1) -> x[n1 R2 + n2]
+// Both inter-step twiddles w_M^{+-n2 k1} are applied by the thread that owns k1: it loads its R2 - 1 factors once
+// per tile and uses them for the three components in both directions (the R1-point steps move no twiddles).
 #include "fe_fft2.cuh"
 #include <stdlib.h>
 
@@ -36,6 +38,8 @@ struct Z2Args {
     int64_t cs, s_z, s_ky, s_g;
     int64_t kcs, k_skz, k_sky, k_sg;
     int pa, pb, pc;   // ky is stored in slot order (k1 pb + k2) pc + k3, ky = k1 + pa k2 + pa pb k3; pa = 0: natural
+    int gs;           // tiles per stored group of kx (1; 2 when a tile is half a 128-byte row): tile group kxg sits at
+                      // (kxg / gs) * s_g + (kxg % gs) * LANES
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
@@ -54,6 +58,13 @@ template <int BYTES> __device__ __forceinline__ void cp_async_n(void* smem, cons
     if constexpr (BYTES == 16) cp_async16(smem, gmem);
     else cp_async8(smem, gmem);
 }
+// x with its sign bit flipped when s = 0x80000000 (integer pipe: keeps the sign changes of the odd tensor
+// components out of the floating-point pipe)
+__device__ __forceinline__ double xorsign(double x, unsigned s)
+{
+    return __hiloint2double(__double2hiint(x) ^ (int)s, __double2loint(x));
+}
+__device__ __forceinline__ float xorsign(float x, unsigned s) { return __uint_as_float(__float_as_uint(x) ^ s); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
@@ -110,7 +121,6 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     using C = ZCfg<T, M, LANES, PRUNE>;
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT1 = C::NT1, TILE = C::TILE, NIN = C::NIN, HZ = C::HZ;
     constexpr int P1 = C::P1, P2 = C::P2;
-    constexpr int NLOAD = PRUNE ? R1 / 2 : R1;
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);
     cx<T>* buf = tw + M;                                            // exchange [3][M][LANES]
     cx<T>* stage = buf + 3 * TILE;                                  // staged input [3][NIN][LANES]
@@ -123,7 +133,8 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         it.tile(a, b, ky);
         int slot = ky;
         if (a.pa) slot = ((ky % a.pa) * a.pb + (ky / a.pa) % a.pb) * a.pc + ky / (a.pa * a.pb);
-        return S + (int64_t)b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)it.kxg * a.s_g;
+        return S + (int64_t)b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)(it.kxg / a.gs) * a.s_g +
+               (it.kxg % a.gs) * LANES;
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
     auto prefetch_tile = [&](const ZIter& it) {
@@ -151,7 +162,8 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         static_assert(LANES * sizeof(T) >= 8 && C::THREADS % OPS_ROW == 0, "a K~ row of a tile must be at least 8 bytes");
         const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
         const int64_t krs = a.k_skz;                                    // stride of kz in the table
-        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)it.kxg * a.k_sg + (int64_t)row0 * krs + q * PER;
+        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)(it.kxg / a.gs) * a.k_sg + (it.kxg % a.gs) * LANES +
+                     (int64_t)row0 * krs + q * PER;
         T* s = kbuf + row0 * LANES + q * PER;
 #pragma unroll
         for (int c6 = 0; c6 < 6; ++c6) {
@@ -184,7 +196,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         nxt.next(a);
         cp_async_wait<1>();                 // this tile's input has landed (the newest group may still be in flight)
         __syncthreads();                    // ... for every thread; also: previous tile's exchange reads are done
-        // ---- forward step 1: tasks (c, n2)
+        // ---- forward step 1: tasks (c, n2): R1-point over n1 (inputs in bit-reversed register order, k1 natural)
 #pragma unroll
         for (int it = 0; it < NT1; ++it) {
             const int task = tp + it * TPP;
@@ -192,28 +204,35 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                 const int c = task / R2, n2 = task % R2;
                 cx<T> w[R1];
                 const cx<T>* src = stage + (c * NIN + n2) * LANES + lane;
-                static_for<NLOAD>([&](auto ic) { w[decltype(ic)::value] = src[decltype(ic)::value * R2 * LANES]; });
-                Dif<T, -1, R1, 0, PRUNE>::run(w);
-                cx<T>* dst = buf + c * TILE + n2 * LANES + lane;
                 static_for<R1>([&](auto pc) {
                     constexpr int p = decltype(pc)::value;
-                    constexpr int k1 = brev<R1>(p);
-                    cx<T> val = w[p];
-                    if constexpr (k1 != 0) val = cmul(val, tw[n2 * k1]);
-                    dst[k1 * P2 * LANES] = val;
+                    constexpr int n1 = brev<R1>(p);
+                    if constexpr (!PRUNE || n1 < R1 / 2) w[p] = src[n1 * R2 * LANES];
                 });
+                DitF<T, -1, R1, 0, PRUNE, false>::run(w);
+                cx<T>* dst = buf + c * TILE + n2 * LANES + lane;
+                static_for<R1>([&](auto kc) { dst[decltype(kc)::value * P2 * LANES] = w[decltype(kc)::value]; });
             }
         }
         __syncthreads();                    // exchange written, staging buffer free
         if (nxt.valid(a)) prefetch_tile(nxt);
         cp_async_commit();                  // group A (possibly empty): input of the next tile
-        // ---- forward step 3 for thread k1 = tp: u[c][p] = P~_c[k1 + R1 brev(p)]
+        // ---- forward step 3 for thread k1 = tp: twiddle, R2-point over n2; u[c][p] = P~_c[k1 + R1 brev(p)]
         const int k1 = tp;
+        cx<T> wk[R2];                       // w_M^{n2 k1}, n2 = 1 .. R2-1 (wk[0] unused)
+        static_for<R2 - 1>([&](auto nc) { wk[decltype(nc)::value + 1] = tw[(decltype(nc)::value + 1) * k1]; });
         cx<T> u[3][R2];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const cx<T>* src = buf + c * TILE + k1 * P2 * LANES + lane;
             static_for<R2>([&](auto nc) { u[c][decltype(nc)::value] = src[decltype(nc)::value * LANES]; });
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            static_for<R2 - 1>([&](auto nc) {
+                constexpr int n2 = decltype(nc)::value + 1;
+                u[c][n2] = cmul(u[c][n2], wk[n2]);
+            });
             Dif<T, -1, R2>::run(u[c]);
         }
         cp_async_wait<1>();                 // K~ of this item has landed (only the group just committed may be pending)
@@ -221,17 +240,17 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         // ---- multiply
         {
             const T esc = (T)(-escale);
-            const T sy = 2 * ky > a.My ? -esc : esc;
+            const unsigned sy = 2 * ky > a.My ? 0x80000000u : 0u;      // sign bits of the odd components
             static_for<R2>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
                 constexpr int k2 = brev<R2>(p);
                 const int kz = k1 + R1 * k2;
                 const int kzm = 2 * kz <= M ? kz : M - kz;
-                const T sz = 2 * kz > M ? (T)-1 : (T)1;
+                const unsigned sz = 2 * kz > M ? 0x80000000u : 0u;
                 const T* kp = kbuf + kzm * LANES + lane;
                 const T Kxx = esc * kp[0], Kyy = esc * kp[HZ * LANES], Kzz = esc * kp[2 * HZ * LANES];
-                const T Kxy = sy * kp[3 * HZ * LANES], Kxz = esc * sz * kp[4 * HZ * LANES];
-                const T Kyz = sy * sz * kp[5 * HZ * LANES];
+                const T Kxy = xorsign(esc * kp[3 * HZ * LANES], sy), Kxz = xorsign(esc * kp[4 * HZ * LANES], sz);
+                const T Kyz = xorsign(esc * kp[5 * HZ * LANES], sy ^ sz);
                 const cx<T> Px = u[0][p], Py = u[1][p], Pz = u[2][p];
                 u[0][p] = {Kxx * Px.x + Kxy * Py.x + Kxz * Pz.x, Kxx * Px.y + Kxy * Py.y + Kxz * Pz.y};
                 u[1][p] = {Kxy * Px.x + Kyy * Py.x + Kyz * Pz.x, Kxy * Px.y + Kyy * Py.y + Kyz * Pz.y};
@@ -241,12 +260,12 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         // ---- inverse step 1: R2-point over k2 (bit-reversed in, natural n2 out), twiddle, exchange
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            Dit<T, +1, R2>::run(u[c]);
+            DitF<T, +1, R2>::run(u[c]);
             cx<T>* dst = buf + c * TILE + k1 * LANES + lane;
             static_for<R2>([&](auto nc) {
                 constexpr int n2 = decltype(nc)::value;
                 cx<T> val = u[c][n2];
-                if constexpr (n2 != 0) val = cmulc(val, tw[n2 * k1]);
+                if constexpr (n2 != 0) val = cmulc(val, wk[n2]);
                 dst[n2 * P1 * LANES] = val;
             });
         }
@@ -261,14 +280,13 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                 const int c = task / R2, n2 = task % R2;
                 cx<T> w[R1];
                 const cx<T>* src = buf + c * TILE + n2 * P1 * LANES + lane;
-                static_for<R1>([&](auto kc) { w[decltype(kc)::value] = src[decltype(kc)::value * LANES]; });
-                Dif<T, +1, R1>::run(w);
+                static_for<R1>([&](auto pc) { w[decltype(pc)::value] = src[brev<R1>(decltype(pc)::value) * LANES]; });
+                DitF<T, +1, R1, 0, false, PRUNE>::run(w);
                 cx<T>* out = base + c * cs + (int64_t)n2 * sa;
-                static_for<R1>([&](auto pc) {
-                    constexpr int p = decltype(pc)::value;
-                    constexpr int n1 = brev<R1>(p);
+                static_for<R1>([&](auto nc) {
+                    constexpr int n1 = decltype(nc)::value;
                     if constexpr (!PRUNE || n1 < R1 / 2) {
-                        if (!PRUNE || R2 * n1 + n2 < a.nz) out[(int64_t)(R2 * n1) * sa] = w[p];
+                        if (!PRUNE || R2 * n1 + n2 < a.nz) out[(int64_t)(R2 * n1) * sa] = w[n1];
                     }
                 });
             }
@@ -319,7 +337,7 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
     const int M = c.plan[2].M;
     constexpr int L128 = 128 / (int)sizeof(v2::cx<T>);      // lanes of a 128-byte row
     v2::Z2Args a{c.tw, members, My, batch, nz, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
-                 kstr[0], kstr[1], kstr[2], kstr[3], perm[0], perm[1], perm[2]};
+                 kstr[0], kstr[1], kstr[2], kstr[3], perm[0], perm[1], perm[2], 1};
     const bool prune = 2 * nz <= M;              // zero-padded axis
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
@@ -329,9 +347,9 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
             // 128-byte rows (one 256-thread block per SM) beat 64-byte rows (two 128-thread blocks) on B200:
             // 0.66 vs 0.80 ms at cfg5a.  FE_B200_ZLANES=4 selects the narrow tile (tuning aid).
             static const int zl = getenv("FE_B200_ZLANES") ? atoi(getenv("FE_B200_ZLANES")) : 0;
-            if (zl == 4 && a.s_g == L128 && a.k_sg == L128) {
-                // half-width tiles (row-major spectra only): twice the groups, half the group stride
-                a.ngroups *= 2; a.s_g /= 2; a.k_sg /= 2;
+            if (zl == 4) {
+                // half-width tiles: twice the groups, two tiles per stored group
+                a.ngroups *= 2; a.gs = 2;
                 return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
             }
             return v2::launch_p<T, 256, L128>(prune, S, Kt, a, st);
