@@ -37,9 +37,10 @@ struct Z2Args {
     int nitems;       // ngroups * (My/2 + 1)
     int64_t cs, s_z, s_ky, s_g;
     int64_t kcs, k_skz, k_sky, k_sg;
-    int pa, pb, pc;   // ky is stored in slot order (k1 pb + k2) pc + k3, ky = k1 + pa k2 + pa pb k3; pa = 0: natural
+    int la, lb, lc;   // ky is stored in slot order (k1 pb + k2) pc + k3, ky = k1 + pa k2 + pa pb k3, with the binary
+                      // logarithms of pa, pb, pc given; la < 0: natural order
     int gs;           // tiles per stored group of kx (1; 2 when a tile is half a 128-byte row): tile group kxg sits at
-                      // (kxg / gs) * s_g + (kxg % gs) * LANES
+                      // (kxg / gs) * s_g + (kxg % gs) * LANES (gs is 1 or 2)
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
@@ -88,30 +89,35 @@ template <typename T, int M, int LANES, bool PRUNE> struct ZCfg {
     static constexpr size_t smem = tw_bytes + ex_bytes + st_bytes + k_bytes;
 };
 
-// position of a block in its sequence of tiles
+// position of a block in its sequence of tiles; advanced without divisions (the loop head is executed by every
+// thread once per tile, and its integer chain is not hidden by anything else)
 struct ZIter {
-    int item, t, nt;          // work item, tile within the item, tiles in the item
-    int kxg, kyh;
-    __device__ __forceinline__ void set_item(int it, const Z2Args& a)
+    int kxg, kyh;             // work item
+    int b, m, nm;             // batch member, mirror index (ky = m ? My - kyh : kyh), mirrors of the item (1 or 2)
+    __device__ __forceinline__ void set_item(int g, int h, const Z2Args& a)
     {
-        item = it;
-        t = 0;
-        kxg = it % a.ngroups;
-        kyh = it / a.ngroups;
-        nt = a.batch * ((kyh == 0 || 2 * kyh == a.My) ? 1 : 2);
+        kxg = g;
+        kyh = h;
+        b = 0;
+        m = 0;
+        nm = (h == 0 || 2 * h == a.My) ? 1 : 2;
     }
-    __device__ __forceinline__ bool valid(const Z2Args& a) const { return item < a.nitems; }
-    __device__ __forceinline__ void next(const Z2Args& a)
+    __device__ __forceinline__ bool valid(const Z2Args& a) const { return 2 * kyh <= a.My; }
+    // dq, dr: quotient and remainder of gridDim.x by a.ngroups
+    __device__ __forceinline__ void next(const Z2Args& a, int dq, int dr)
     {
-        if (++t >= nt) set_item(item + gridDim.x, a);
+        if (++m < nm) return;
+        m = 0;
+        if (++b < a.batch) return;
+        int g = kxg + dr, h = kyh + dq;
+        if (g >= a.ngroups) {
+            g -= a.ngroups;
+            ++h;
+        }
+        set_item(g, h, a);
     }
-    // batch member and signed ky of the current tile
-    __device__ __forceinline__ void tile(const Z2Args& a, int& b, int& ky) const
-    {
-        const int nm = nt / a.batch;
-        b = t / nm;
-        ky = (t % nm) ? a.My - kyh : kyh;
-    }
+    __device__ __forceinline__ bool same_item(const ZIter& o) const { return kxg == o.kxg && kyh == o.kyh; }
+    __device__ __forceinline__ int ky(const Z2Args& a) const { return m ? a.My - kyh : kyh; }
 };
 
 template <typename T, int M, int LANES, bool PRUNE>
@@ -129,12 +135,13 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     const int64_t sa = a.s_z, cs = a.cs, kcs = a.kcs;
 
     auto tile_base = [&](const ZIter& it) -> cx<T>* {
-        int b, ky;
-        it.tile(a, b, ky);
+        const int ky = it.ky(a);
         int slot = ky;
-        if (a.pa) slot = ((ky % a.pa) * a.pb + (ky / a.pa) % a.pb) * a.pc + ky / (a.pa * a.pb);
-        return S + (int64_t)b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)(it.kxg / a.gs) * a.s_g +
-               (it.kxg % a.gs) * LANES;
+        if (a.la >= 0)
+            slot = ((ky & ((1 << a.la) - 1)) << (a.lb + a.lc)) | (((ky >> a.la) & ((1 << a.lb) - 1)) << a.lc) |
+                   (ky >> (a.la + a.lb));
+        return S + (int64_t)it.b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)(it.kxg >> (a.gs - 1)) * a.s_g +
+               (it.kxg & (a.gs - 1)) * LANES;
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
     auto prefetch_tile = [&](const ZIter& it) {
@@ -162,7 +169,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         static_assert(LANES * sizeof(T) >= 8 && C::THREADS % OPS_ROW == 0, "a K~ row of a tile must be at least 8 bytes");
         const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
         const int64_t krs = a.k_skz;                                    // stride of kz in the table
-        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)(it.kxg / a.gs) * a.k_sg + (it.kxg % a.gs) * LANES +
+        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)(it.kxg >> (a.gs - 1)) * a.k_sg + (it.kxg & (a.gs - 1)) * LANES +
                      (int64_t)row0 * krs + q * PER;
         T* s = kbuf + row0 * LANES + q * PER;
 #pragma unroll
@@ -175,8 +182,9 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     };
 
     ZIter cur;
-    cur.set_item(blockIdx.x, a);
+    cur.set_item(blockIdx.x % a.ngroups, blockIdx.x / a.ngroups, a);
     if (!cur.valid(a)) return;
+    const int dq = gridDim.x / a.ngroups, dr = gridDim.x % a.ngroups;
     if (PRUNE && a.nz < NIN) {              // padding rows inside the staged half: cleared once, never written again
         for (int e = threadIdx.x; e < 3 * NIN * LANES; e += C::THREADS) stage[e] = cx<T>{0, 0};
         __syncthreads();
@@ -188,12 +196,11 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, C::THREADS);
 
     while (cur.valid(a)) {
-        int b, ky;
-        cur.tile(a, b, ky);
+        const int ky = cur.ky(a);
         cx<T>* base = tile_base(cur) + lane;
-        const double escale = a.members[b].escale;      // issued here, consumed after the forward transform
+        const double escale = a.members[cur.b].escale;  // issued here, consumed after the forward transform
         ZIter nxt = cur;
-        nxt.next(a);
+        nxt.next(a, dq, dr);
         cp_async_wait<1>();                 // this tile's input has landed (the newest group may still be in flight)
         __syncthreads();                    // ... for every thread; also: previous tile's exchange reads are done
         // ---- forward step 1: tasks (c, n2): R1-point over n1 (inputs in bit-reversed register order, k1 natural)
@@ -270,7 +277,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
             });
         }
         __syncthreads();                    // exchange written; every thread is past the multiply: K~ buffer free
-        if (nxt.valid(a) && nxt.item != cur.item) prefetch_k(nxt);
+        if (nxt.valid(a) && !nxt.same_item(cur)) prefetch_k(nxt);
         cp_async_commit();                  // group B (possibly empty): K~ of the next item
         // ---- inverse step 2: tasks (c, n2): R1-point over k1, rows n1 R2 + n2 (n1 < R1/2 when pruned) stored
 #pragma unroll
@@ -314,6 +321,7 @@ static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
         nblocks = sms * (per > 0 ? per : 1);
     }
     a.nitems = a.ngroups * (a.My / 2 + 1);
+    if (a.gs != 1 && a.gs != 2) return cudaErrorInvalidValue;
     const int grid = a.nitems < nblocks ? a.nitems : nblocks;
     k2_zmul<T, M, LANES, PRUNE><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a);
     return cudaGetLastError();
@@ -336,8 +344,17 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
 {
     const int M = c.plan[2].M;
     constexpr int L128 = 128 / (int)sizeof(v2::cx<T>);      // lanes of a 128-byte row
+    // slot order of ky: radices of the three-level y pass (powers of two), or natural order
+    int lg[3] = {-1, 0, 0};
+    if (perm[0]) {
+        for (int i = 0; i < 3; ++i) {
+            if (perm[i] <= 0 || (perm[i] & (perm[i] - 1))) return cudaErrorInvalidValue;
+            lg[i] = 0;
+            while ((1 << lg[i]) < perm[i]) ++lg[i];
+        }
+    }
     v2::Z2Args a{c.tw, members, My, batch, nz, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
-                 kstr[0], kstr[1], kstr[2], kstr[3], perm[0], perm[1], perm[2], 1};
+                 kstr[0], kstr[1], kstr[2], kstr[3], lg[0], lg[1], lg[2], 1};
     const bool prune = 2 * nz <= M;              // zero-padded axis
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
