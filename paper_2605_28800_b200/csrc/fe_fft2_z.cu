@@ -246,7 +246,6 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         __syncthreads();                    // ... for every thread; exchange fully read
         // ---- multiply
         {
-            const T esc = (T)(-escale);
             const unsigned sy = 2 * ky > a.My ? 0x80000000u : 0u;      // sign bits of the odd components
             static_for<R2>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
@@ -255,26 +254,35 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                 const int kzm = 2 * kz <= M ? kz : M - kz;
                 const unsigned sz = 2 * kz > M ? 0x80000000u : 0u;
                 const T* kp = kbuf + kzm * LANES + lane;
-                const T Kxx = esc * kp[0], Kyy = esc * kp[HZ * LANES], Kzz = esc * kp[2 * HZ * LANES];
-                const T Kxy = xorsign(esc * kp[3 * HZ * LANES], sy), Kxz = xorsign(esc * kp[4 * HZ * LANES], sz);
-                const T Kyz = xorsign(esc * kp[5 * HZ * LANES], sy ^ sz);
+                const T Kxx = kp[0], Kyy = kp[HZ * LANES], Kzz = kp[2 * HZ * LANES];
+                const T Kxy = xorsign(kp[3 * HZ * LANES], sy), Kxz = xorsign(kp[4 * HZ * LANES], sz);
+                const T Kyz = xorsign(kp[5 * HZ * LANES], sy ^ sz);
                 const cx<T> Px = u[0][p], Py = u[1][p], Pz = u[2][p];
                 u[0][p] = {Kxx * Px.x + Kxy * Py.x + Kxz * Pz.x, Kxx * Px.y + Kxy * Py.y + Kxz * Pz.y};
                 u[1][p] = {Kxy * Px.x + Kyy * Py.x + Kyz * Pz.x, Kxy * Px.y + Kyy * Py.y + Kyz * Pz.y};
                 u[2][p] = {Kxz * Px.x + Kyz * Py.x + Kzz * Pz.x, Kxz * Px.y + Kyz * Py.y + Kzz * Pz.y};
             });
         }
-        // ---- inverse step 1: R2-point over k2 (bit-reversed in, natural n2 out), twiddle, exchange
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            DitF<T, +1, R2>::run(u[c]);
-            cx<T>* dst = buf + c * TILE + k1 * LANES + lane;
-            static_for<R2>([&](auto nc) {
-                constexpr int n2 = decltype(nc)::value;
-                cx<T> val = u[c][n2];
-                if constexpr (n2 != 0) val = cmulc(val, wk[n2]);
-                dst[n2 * P1 * LANES] = val;
+        // ---- inverse step 1: R2-point over k2 (bit-reversed in, natural n2 out), twiddle, exchange.  The factor
+        // -escale of Eq. 6 rides on the twiddles (2 (R2 - 1) + 6 multiplications instead of 6 R2 on the tensor).
+        {
+            const T esc = (T)(-escale);
+            static_for<R2 - 1>([&](auto nc) {
+                constexpr int n2 = decltype(nc)::value + 1;
+                wk[n2] = {esc * wk[n2].x, esc * wk[n2].y};
             });
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                DitF<T, +1, R2>::run(u[c]);
+                cx<T>* dst = buf + c * TILE + k1 * LANES + lane;
+                static_for<R2>([&](auto nc) {
+                    constexpr int n2 = decltype(nc)::value;
+                    cx<T> val = u[c][n2];
+                    if constexpr (n2 != 0) val = cmulc(val, wk[n2]);
+                    else val = {esc * val.x, esc * val.y};
+                    dst[n2 * P1 * LANES] = val;
+                });
+            }
         }
         __syncthreads();                    // exchange written; every thread is past the multiply: K~ buffer free
         if (nxt.valid(a) && !nxt.same_item(cur)) prefetch_k(nxt);
