@@ -291,10 +291,40 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
             }
         }
     }
+    // Inter-level twiddles of this thread's tasks.  They do not depend on the tile, and a load from the table
+    // cannot be moved above a store to the tile by the compiler (both live in shared memory), so loading them
+    // where they are used puts one shared-memory latency between every two stores.  With 256 threads they stay in
+    // registers for the whole kernel; the 512-thread variant reloads them at the top of every tile.
+    static_assert(TPP % RB == 0 && TPP % RC == 0, "digits of a task must not depend on the task round");
+    constexpr bool HOIST = THREADS <= 256;
+    constexpr int NWA = DIR < 0 ? NTA / TPP : NTB / TPP;
+    cx<T> w1[NWA][8];                    // forward: level A, tw[j k1];       inverse: level B', tw[(n3 + RC n2) k1]
+    cx<T> w2[8];                         // forward: level B, tw[RA n3 k2];   inverse: level C', tw[RA n3 k2]
+    auto load_tw = [&]() {
+        if (DIR < 0) {
+#pragma unroll
+            for (int it = 0; it < NTA / TPP; ++it) {
+                const int j = tp + it * TPP;
+                static_for<RA - 1>([&](auto kc) { w1[it][decltype(kc)::value + 1] = tw[j * (decltype(kc)::value + 1)]; });
+            }
+            const int n3 = tp % RC;
+            static_for<RB - 1>([&](auto kc) { w2[decltype(kc)::value + 1] = tw[RA * n3 * (decltype(kc)::value + 1)]; });
+        } else {
+            const int k2 = tp % RB;
+            static_for<RC - 1>([&](auto nc) { w2[decltype(nc)::value + 1] = tw[RA * (decltype(nc)::value + 1) * k2]; });
+#pragma unroll
+            for (int it = 0; it < NTB / TPP; ++it) {
+                const int tb = tp + it * TPP, n3 = tb % RC, k1 = tb / RC;
+                static_for<RB>([&](auto nc) { w1[it][decltype(nc)::value] = tw[(n3 + RC * decltype(nc)::value) * k1]; });
+            }
+        }
+    };
+    if (HOIST) load_tw();
     int i = 0;
     for (int t = t0; t < a.ntiles; t += dt, ++i) {
         const int b = i % NB;
         cx<T>* buf = bufs + b * TILE + lane;
+        if (!HOIST) load_tw();
         mbar_wait(&bars[b], (unsigned)((i / NB) & 1));
         if (PIN && a.n_keep < M / 2) {
             // the zero padding below M/2 is not part of the tile in memory: clear the rows the previous tile left there
@@ -314,7 +344,7 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
                     constexpr int p = decltype(pc)::value;
                     constexpr int k1 = brev<RA>(p);
                     cx<T> val = u[p];
-                    if constexpr (k1 != 0) val = cmul(val, tw[j * k1]);
+                    if constexpr (k1 != 0) val = cmul(val, w1[it][k1]);
                     col[k1 * RB * RC * LANES] = val;
                 });
             }
@@ -331,7 +361,7 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
                     constexpr int p = decltype(pc)::value;
                     constexpr int k2 = brev<RB>(p);
                     cx<T> val = u[p];
-                    if constexpr (k2 != 0) val = cmul(val, tw[RA * n3 * k2]);
+                    if constexpr (k2 != 0) val = cmul(val, w2[k2]);
                     col[k2 * RC * LANES] = val;
                 });
             }
@@ -359,7 +389,7 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
                     constexpr int p = decltype(pc)::value;
                     constexpr int n3 = brev<RC>(p);
                     cx<T> val = u[p];
-                    if constexpr (n3 != 0) val = cmulc(val, tw[RA * n3 * k2]);
+                    if constexpr (n3 != 0) val = cmulc(val, w2[n3]);
                     col[n3 * LANES] = val;
                 });
             }
@@ -375,7 +405,7 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
                 static_for<RB>([&](auto pc) {
                     constexpr int p = decltype(pc)::value;
                     constexpr int n2 = brev<RB>(p);
-                    col[n2 * RC * LANES] = cmulc(u[p], tw[(n3 + RC * n2) * k1]);
+                    col[n2 * RC * LANES] = cmulc(u[p], w1[it][n2]);
                 });
             }
             __syncthreads();
