@@ -110,7 +110,7 @@ template <typename T, int M, bool PRUNE>
 __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __restrict__ in, T* __restrict__ out, X2Args a)
 {
     using C = XCfg<M>;
-    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT3 = R1 / TPP;
+    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT3 = R1 / TPP, TWG = R1 < 8 ? R1 : 8;
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);
     cx<T>* tws = tw + M;
     cx<T>* buf = tws + M;
@@ -141,12 +141,23 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
         v[j1] = {ex - oy, ey + ox};
     });
     Dif<T, +1, R1>::run(v);
-    static_for<R1>([&](auto pc) {
-        constexpr int p = decltype(pc)::value;
-        constexpr int o1 = brev<R1>(p);
-        cx<T> val = v[p];
-        if constexpr (o1 != 0) val = cmulc(val, tw[o1 * R2 + tp]);
-        rb[o1 * (R2 + 1) + tp] = val;
+    // twiddles are fetched in groups of TWG ahead of the stores they feed: a load from the table cannot be moved
+    // above a store to the row buffer by the compiler (both are shared memory).  (The forward kernel is bound by
+    // shared-memory throughput, not latency, and is faster with the loads left where they are used.)
+    static_for<R1 / TWG>([&](auto gc) {
+        constexpr int g = decltype(gc)::value;
+        cx<T> w[TWG];
+        static_for<TWG>([&](auto qc) {
+            constexpr int o1 = brev<R1>(g * TWG + decltype(qc)::value);
+            if constexpr (o1 != 0) w[decltype(qc)::value] = tw[o1 * R2 + tp];
+        });
+        static_for<TWG>([&](auto qc) {
+            constexpr int p = g * TWG + decltype(qc)::value;
+            constexpr int o1 = brev<R1>(p);
+            cx<T> val = v[p];
+            if constexpr (o1 != 0) val = cmulc(val, w[decltype(qc)::value]);
+            rb[o1 * (R2 + 1) + tp] = val;
+        });
     });
     __syncthreads();
 #pragma unroll
