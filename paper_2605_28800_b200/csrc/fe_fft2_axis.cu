@@ -43,12 +43,23 @@ k2_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis2Args a)
     load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, LANES * TPP);
     __syncthreads();
     Dif<T, DIR, R1, 0, PIN>::run(v);
-    static_for<R1>([&](auto pc) {
-        constexpr int p = decltype(pc)::value;
-        constexpr int k1 = brev<R1>(p);
-        cx<T> val = v[p];
-        if constexpr (k1 != 0) val = cmuld<T, DIR>(val, tw[tp * k1]);
-        buf[(k1 * R2 + tp) * LANES + lane] = val;
+    // twiddles are fetched in groups ahead of the stores they feed (a shared-memory load cannot be moved above a
+    // shared-memory store by the compiler)
+    constexpr int TWG = R1 < 8 ? R1 : 8;
+    static_for<R1 / TWG>([&](auto gc) {
+        constexpr int g = decltype(gc)::value;
+        cx<T> w[TWG];
+        static_for<TWG>([&](auto qc) {
+            constexpr int k1 = brev<R1>(g * TWG + decltype(qc)::value);
+            if constexpr (k1 != 0) w[decltype(qc)::value] = tw[tp * k1];
+        });
+        static_for<TWG>([&](auto qc) {
+            constexpr int p = g * TWG + decltype(qc)::value;
+            constexpr int k1 = brev<R1>(p);
+            cx<T> val = v[p];
+            if constexpr (k1 != 0) val = cmuld<T, DIR>(val, w[decltype(qc)::value]);
+            buf[(k1 * R2 + tp) * LANES + lane] = val;
+        });
     });
     __syncthreads();
     // step 3: thread k1 = tp (+ TPP ...) runs the R2-point transform over n2
