@@ -331,6 +331,18 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
         }
     };
     if (HOIST) load_tw();
+    // The buffer of tile i-1 is reused for tile i+2: its store must have finished reading shared memory.  Issued
+    // by thread 0 after the first level of tile i (the store of tile i-1 is the newest bulk group then), which gives
+    // the load two thirds of a tile more lead than issuing it behind the store of tile i.
+    auto prefetch_next = [&](int t, int i) {
+        const int tn = t + 2 * dt;
+        if (tn < a.ntiles) {
+            bulk_wait_read<0>();
+            const int bn = (i + 2) % NB;
+            mbar_expect_tx(&bars[bn], in_bytes);
+            bulk_load(bufs + bn * TILE, in_ptr(tn), in_bytes, &bars[bn]);
+        }
+    };
     int i = 0;
     for (int t = t0; t < a.ntiles; t += dt, ++i) {
         const int b = i % NB;
@@ -360,6 +372,7 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
                 });
             }
             __syncthreads();
+            if (threadIdx.x == 0) prefetch_next(t, i);
             // ---- B: task (k1, n3), slots k1 RB RC + n3 + RC n2
 #pragma unroll
             for (int it = 0; it < NTB / TPP; ++it) {
@@ -405,6 +418,7 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
                 });
             }
             __syncthreads();
+            if (threadIdx.x == 0) prefetch_next(t, i);
             // ---- B': task (k1, n3), slots k1 RB RC + n3 + RC k2 -> n2
 #pragma unroll
             for (int it = 0; it < NTB / TPP; ++it) {
@@ -439,14 +453,6 @@ k4_axis(const cx<T>* __restrict__ in, cx<T>* __restrict__ out, Axis4Args a)
         __syncthreads();
         if (threadIdx.x == 0) {
             bulk_store(out_ptr(t), bufs + b * TILE, out_bytes);
-            // the buffer of tile i-1 is reused for tile i+2: its store must have finished reading shared memory
-            const int tn = t + 2 * dt;
-            if (tn < a.ntiles) {
-                bulk_wait_read<1>();
-                const int bn = (i + 2) % NB;
-                mbar_expect_tx(&bars[bn], in_bytes);
-                bulk_load(bufs + bn * TILE, in_ptr(tn), in_bytes, &bars[bn]);
-            }
         }
     }
     if (threadIdx.x == 0) bulk_wait_read<0>();
