@@ -41,21 +41,26 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
     cx<T>* tws = tw + M;                              // w_2M^k, k < M
     cx<T>* buf = tws + M;
     const int tp = threadIdx.x % TPP, rl = threadIdx.x / TPP;
-    const int64_t row = (int64_t)blockIdx.x * C::ROWS + rl;
-    const bool live = row < a.nrows;
     cx<T>* rb = buf + rl * C::RPITCH;
-
-    cx<T> v[R1];
     constexpr int NLOAD = PRUNE ? R1 / 2 : R1;
-    if (live) {
-        const cx<T>* src = reinterpret_cast<const cx<T>*>(in + row * a.real_rs) + tp;
-        static_for<NLOAD>([&](auto ic) {
-            constexpr int n1 = decltype(ic)::value;
-            v[n1] = (!PRUNE || tp + R2 * n1 < a.nc) ? src[R2 * n1] : cx<T>{0, 0};
-        });
-    } else {
-        static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = cx<T>{0, 0}; });
-    }
+    // persistent: a block walks over groups of ROWS rows; the real input of the next group is fetched into registers
+    // before the current group is transformed, so the global-load latency hides behind a whole group of work
+    const int64_t ngroups = (a.nrows + C::ROWS - 1) / C::ROWS;
+    auto fetch = [&](int64_t grp, cx<T>* dst) {
+        const int64_t row = grp * C::ROWS + rl;
+        if (grp < ngroups && row < a.nrows) {
+            const cx<T>* src = reinterpret_cast<const cx<T>*>(in + row * a.real_rs) + tp;
+            static_for<NLOAD>([&](auto ic) {
+                constexpr int n1 = decltype(ic)::value;
+                dst[n1] = (!PRUNE || tp + R2 * n1 < a.nc) ? src[R2 * n1] : cx<T>{0, 0};
+            });
+        } else {
+            static_for<NLOAD>([&](auto ic) { dst[decltype(ic)::value] = cx<T>{0, 0}; });
+        }
+    };
+    constexpr bool PF = PRUNE;           // a full-length row (periodic axis) leaves no registers for the prefetch
+    cx<T> vn[PF ? NLOAD : 1];
+    if constexpr (PF) fetch(blockIdx.x, vn);
     {
         const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
         // tw[k1 * R2 + n2] = w_M^(n2 k1): the R2 threads of a row read consecutive entries (no bank conflicts)
@@ -65,44 +70,56 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xfwd(const T* __rest
         }
     }
     __syncthreads();
-    Dif<T, -1, R1, 0, PRUNE>::run(v);
-    static_for<R1>([&](auto pc) {
-        constexpr int p = decltype(pc)::value;
-        constexpr int k1 = brev<R1>(p);
-        cx<T> val = v[p];
-        if constexpr (k1 != 0) val = cmul(val, tw[k1 * R2 + tp]);
-        rb[k1 * (R2 + 1) + tp] = val;
-    });
-    __syncthreads();
-    cx<T> u[NT3][R2];
-#pragma unroll
-    for (int it = 0; it < NT3; ++it) {
-        const int k1 = tp + it * TPP;
-        static_for<R2>([&](auto nc) { u[it][decltype(nc)::value] = rb[k1 * (R2 + 1) + decltype(nc)::value]; });
-        Dif<T, -1, R2>::run(u[it]);
-    }
-    __syncthreads();     // exchange layout fully read; reuse the row buffer in natural order
-#pragma unroll
-    for (int it = 0; it < NT3; ++it) {
-        const int k1 = tp + it * TPP;
-        static_for<R2>([&](auto pc) {
-            constexpr int p = decltype(pc)::value;
-            rb[k1 + R1 * brev<R2>(p)] = u[it][p];
-        });
-    }
-    __syncthreads();
-    if (live) {
-        cx<T>* dst = out + spec_row(a, row);
-        for (int k = tp; k <= M / 2; k += TPP) {
-            const cx<T> Zk = rb[k], Zn = rb[(M - k) & (M - 1)];
-            const T ex = (T)0.5 * (Zk.x + Zn.x), ey = (T)0.5 * (Zk.y - Zn.y);
-            const T ox = (T)0.5 * (Zk.y + Zn.y), oy = (T)-0.5 * (Zk.x - Zn.x);
-            const cx<T> w = tws[k];
-            // X[k] = Xe + w Xo;  X[M-k] = conj(Xe) - conj(w Xo)   (w_2M^(M-k) = -conj(w_2M^k), Xo(M-k) = conj Xo(k))
-            const T px = ox * w.x - oy * w.y, py = ox * w.y + oy * w.x;
-            dst[spec_off(a, k)] = {ex + px, ey + py};
-            dst[spec_off(a, M - k)] = {ex - px, py - ey};
+    for (int64_t grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const int64_t row = grp * C::ROWS + rl;
+        const bool live = row < a.nrows;
+        cx<T> v[R1];
+        if constexpr (PF) {
+            static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = vn[decltype(ic)::value]; });
+            fetch(grp + gridDim.x, vn);
+        } else {
+            fetch(grp, v);
         }
+        Dif<T, -1, R1, 0, PRUNE>::run(v);
+        static_for<R1>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int k1 = brev<R1>(p);
+            cx<T> val = v[p];
+            if constexpr (k1 != 0) val = cmul(val, tw[k1 * R2 + tp]);
+            rb[k1 * (R2 + 1) + tp] = val;
+        });
+        __syncthreads();
+        cx<T> u[NT3][R2];
+#pragma unroll
+        for (int it = 0; it < NT3; ++it) {
+            const int k1 = tp + it * TPP;
+            static_for<R2>([&](auto nc) { u[it][decltype(nc)::value] = rb[k1 * (R2 + 1) + decltype(nc)::value]; });
+            Dif<T, -1, R2>::run(u[it]);
+        }
+        __syncthreads();     // exchange layout fully read; reuse the row buffer in natural order
+#pragma unroll
+        for (int it = 0; it < NT3; ++it) {
+            const int k1 = tp + it * TPP;
+            static_for<R2>([&](auto pc) {
+                constexpr int p = decltype(pc)::value;
+                rb[k1 + R1 * brev<R2>(p)] = u[it][p];
+            });
+        }
+        __syncthreads();
+        if (live) {
+            cx<T>* dst = out + spec_row(a, row);
+            for (int k = tp; k <= M / 2; k += TPP) {
+                const cx<T> Zk = rb[k], Zn = rb[(M - k) & (M - 1)];
+                const T ex = (T)0.5 * (Zk.x + Zn.x), ey = (T)0.5 * (Zk.y - Zn.y);
+                const T ox = (T)0.5 * (Zk.y + Zn.y), oy = (T)-0.5 * (Zk.x - Zn.x);
+                const cx<T> w = tws[k];
+                // X[k] = Xe + w Xo;  X[M-k] = conj(Xe) - conj(w Xo)   (w_2M^(M-k) = -conj(w_2M^k), Xo(M-k) = conj Xo(k))
+                const T px = ox * w.x - oy * w.y, py = ox * w.y + oy * w.x;
+                dst[spec_off(a, k)] = {ex + px, ey + py};
+                dst[spec_off(a, M - k)] = {ex - px, py - ey};
+            }
+        }
+        __syncthreads();     // row buffer fully read before the next group's exchange is written
     }
 }
 
@@ -192,7 +209,18 @@ static cudaError_t launch_one(const void* in, void* out, const X2Args& a, cudaSt
             if (e != cudaSuccess) return e;
             configured = true;
         }
-        k2_xfwd<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
+        // persistent: as many blocks as fit on the device (rows are visited with a grid stride)
+        static int nblocks = 0;
+        if (!nblocks) {
+            int dev = 0, sms = 0, per = 0;
+            cudaError_t e;
+            if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+            if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+            if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k2_xfwd<T, M, PRUNE>, 256, smem)) != cudaSuccess) return e;
+            nblocks = sms * (per > 0 ? per : 1);
+        }
+        const dim3 pgrid(grid.x < (unsigned)nblocks ? grid.x : (unsigned)nblocks);
+        k2_xfwd<T, M, PRUNE><<<pgrid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
     } else {
         if (!configured) {
             cudaError_t e = cudaFuncSetAttribute(k2_xinv<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
