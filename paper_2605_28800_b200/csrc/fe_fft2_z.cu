@@ -161,13 +161,16 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                     cp_async_n<CB>(s + (c * NIN + j * RSTEP) * LANES, g + c * cs + (int64_t)(j * RSTEP) * sa);
         }
     };
-    auto prefetch_k = [&](const ZIter& it) {
+    // K~ tile of an item, copied by the NTH threads [T0, T0 + NTH) of the block
+    auto prefetch_k = [&](const ZIter& it, auto nth_c, auto t0_c) {
+        constexpr int NTH = decltype(nth_c)::value, T0 = decltype(t0_c)::value;
         constexpr int CB = LANES * (int)sizeof(T) < 16 ? 8 : 16;
         constexpr int PER = CB / (int)sizeof(T);
         constexpr int OPS_ROW = LANES / PER;
-        constexpr int RSTEP = C::THREADS / OPS_ROW;
-        static_assert(LANES * sizeof(T) >= 8 && C::THREADS % OPS_ROW == 0, "a K~ row of a tile must be at least 8 bytes");
-        const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
+        constexpr int RSTEP = NTH / OPS_ROW;
+        static_assert(LANES * sizeof(T) >= 8 && NTH % OPS_ROW == 0, "a K~ row of a tile must be at least 8 bytes");
+        const int tid = (int)threadIdx.x - T0;
+        const int q = tid % OPS_ROW, row0 = tid / OPS_ROW;
         const int64_t krs = a.k_skz;                                    // stride of kz in the table
         const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)(it.kxg >> (a.gs - 1)) * a.k_sg + (it.kxg & (a.gs - 1)) * LANES +
                      (int64_t)row0 * krs + q * PER;
@@ -180,6 +183,10 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                     cp_async_n<CB>(s + (c6 * HZ + j * RSTEP) * LANES, g + c6 * kcs + (int64_t)(j * RSTEP) * krs);
         }
     };
+    using ic_all = std::integral_constant<int, C::THREADS>;
+    using ic_zero = std::integral_constant<int, 0>;
+    // threads without a task in the R1-point steps (TPP > 3 R2): they fetch the next K~ tile during inverse step 2
+    constexpr int NIDLE = NT1 == 1 && 3 * R2 < TPP ? (TPP - 3 * R2) * LANES : 0;
 
     ZIter cur;
     cur.set_item(blockIdx.x % a.ngroups, blockIdx.x / a.ngroups, a);
@@ -191,7 +198,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     }
     prefetch_tile(cur);
     cp_async_commit();                      // group A: input of the first tile
-    prefetch_k(cur);
+    prefetch_k(cur, ic_all{}, ic_zero{});
     cp_async_commit();                      // group B: K~ of the first item
     load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, C::THREADS);
 
@@ -285,7 +292,14 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
             }
         }
         __syncthreads();                    // exchange written; every thread is past the multiply: K~ buffer free
-        if (nxt.valid(a) && !nxt.same_item(cur)) prefetch_k(nxt);
+        if (nxt.valid(a) && !nxt.same_item(cur)) {
+            if constexpr (NIDLE > 0) {
+                if (tp >= 3 * R2)
+                    prefetch_k(nxt, std::integral_constant<int, NIDLE>{}, std::integral_constant<int, 3 * R2 * LANES>{});
+            } else {
+                prefetch_k(nxt, ic_all{}, ic_zero{});
+            }
+        }
         cp_async_commit();                  // group B (possibly empty): K~ of the next item
         // ---- inverse step 2: tasks (c, n2): R1-point over k1, rows n1 R2 + n2 (n1 < R1/2 when pruned) stored
 #pragma unroll
