@@ -144,14 +144,14 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                (it.kxg & (a.gs - 1)) * LANES;
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
-    auto prefetch_tile = [&](const ZIter& it) {
+    auto prefetch_tile = [&](const cx<T>* tb) {
         constexpr int CB = LANES * (int)sizeof(cx<T>) < 16 ? 8 : 16;   // bytes per copy
         constexpr int PER = CB / (int)sizeof(cx<T>);                    // complex elements per copy
         constexpr int OPS_ROW = LANES / PER;                            // copies per row
         constexpr int RSTEP = C::THREADS / OPS_ROW;                     // rows covered by one sweep of the block
         static_assert(C::THREADS % OPS_ROW == 0 && NIN % RSTEP == 0, "tile copy must be regular");
         const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
-        const cx<T>* g = tile_base(it) + (int64_t)row0 * sa + q * PER;
+        const cx<T>* g = tb + (int64_t)row0 * sa + q * PER;
         cx<T>* s = stage + row0 * LANES + q * PER;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -196,7 +196,8 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         for (int e = threadIdx.x; e < 3 * NIN * LANES; e += C::THREADS) stage[e] = cx<T>{0, 0};
         __syncthreads();
     }
-    prefetch_tile(cur);
+    cx<T>* cur_base = tile_base(cur);       // carried from the prefetch of a tile to its turn in the loop
+    prefetch_tile(cur_base);
     cp_async_commit();                      // group A: input of the first tile
     prefetch_k(cur, ic_all{}, ic_zero{});
     cp_async_commit();                      // group B: K~ of the first item
@@ -204,7 +205,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
 
     while (cur.valid(a)) {
         const int ky = cur.ky(a);
-        cx<T>* base = tile_base(cur) + lane;
+        cx<T>* base = cur_base + lane;
         const double escale = a.members[cur.b].escale;  // issued here, consumed after the forward transform
         ZIter nxt = cur;
         nxt.next(a, dq, dr);
@@ -229,7 +230,10 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
             }
         }
         __syncthreads();                    // exchange written, staging buffer free
-        if (nxt.valid(a)) prefetch_tile(nxt);
+        if (nxt.valid(a)) {
+            cur_base = tile_base(nxt);
+            prefetch_tile(cur_base);
+        }
         cp_async_commit();                  // group A (possibly empty): input of the next tile
         // ---- forward step 3 for thread k1 = tp: twiddle, R2-point over n2; u[c][p] = P~_c[k1 + R1 brev(p)]
         const int k1 = tp;
