@@ -77,6 +77,7 @@ void orc_landau_dfdp(const orc_landau* m, const double* P, double* out)
 void orc_landau_field(const orc_landau* mats, const uint8_t* matmap, int64_t N,
                       const double* P, double* E)
 {
+#pragma omp parallel for schedule(static)
     for (int64_t r = 0; r < N; ++r) {
         const orc_landau* m = &mats[matmap ? matmap[r] : 0];
         double p[3] = { P[r], P[N + r], P[2 * N + r] }, d[3] = { 0, 0, 0 };
@@ -181,6 +182,7 @@ void orc_grad_field(const int* n, const double* d, const int* periodic, const ui
                     { periodic[0], periodic[1], periodic[2] }, act, P };
     double Gm = G12 + G44 - G44p;
     int64_t N = (int64_t)n[0] * n[1] * n[2];
+#pragma omp parallel for collapse(2) schedule(static)
     for (int z = 0; z < n[2]; ++z)
         for (int y = 0; y < n[1]; ++y)
             for (int x = 0; x < n[0]; ++x) {

@@ -234,21 +234,38 @@ def circular_kernel(p: Problem, K: np.ndarray) -> np.ndarray:
     return box
 
 
-def field_fft(p: Problem, K: np.ndarray, P: np.ndarray, box_hat: Optional[np.ndarray] = None) -> np.ndarray:
+def _fftn(a: np.ndarray, axes, workers: Optional[int]):
+    """The library FFT used as one step of O8: numpy.fft, or -- when the caller asks for host threads (bench.py's
+    all-cores CPU baseline) -- scipy.fft with that many workers.  Same transform, same padding."""
+    if workers is None:
+        return np.fft.fftn(a, axes=axes)
+    import scipy.fft
+    return scipy.fft.fftn(a, axes=axes, workers=workers)
+
+
+def _ifftn(a: np.ndarray, workers: Optional[int]):
+    if workers is None:
+        return np.fft.ifftn(a)
+    import scipy.fft
+    return scipy.fft.ifftn(a, workers=workers)
+
+
+def field_fft(p: Problem, K: np.ndarray, P: np.ndarray, box_hat: Optional[np.ndarray] = None,
+              workers: Optional[int] = None) -> np.ndarray:
     """O8: E_elec = -scale * IFFT( FFT(K_box) * FFT(P zero-padded) ), cropped.  Complex transforms
     of the whole padded box; the result's imaginary part is rounding noise and is dropped."""
     nx, ny, nz = p.n
     m = [p.n[a] if p.periodic[a] else 2 * p.n[a] for a in range(3)]
     if box_hat is None:
-        box_hat = np.fft.fftn(circular_kernel(p, K), axes=(1, 2, 3))
+        box_hat = _fftn(circular_kernel(p, K), (1, 2, 3), workers)
     Pp = np.zeros((3, m[2], m[1], m[0]))
     Pp[:, :nz, :ny, :nx] = P
-    Ph = np.fft.fftn(Pp, axes=(1, 2, 3))
+    Ph = _fftn(Pp, (1, 2, 3), workers)
     scale = 1.0 / (p.g.eps0 * p.g.epsB)
     E = np.empty((3, nz, ny, nx))
     for i in range(3):
         acc = sum(box_hat[_CIDX[i][j]] * Ph[j] for j in range(3))
-        E[i] = -scale * np.fft.ifftn(acc).real[:nz, :ny, :nx]
+        E[i] = -scale * _ifftn(acc, workers).real[:nz, :ny, :nx]
     return E
 
 
@@ -268,10 +285,12 @@ RK45_B4 = (2825.0 / 27648.0, 0.0, 18575.0 / 48384.0, 13525.0 / 55296.0, 277.0 / 
 class Oracle:
     """RHS / step / energy of one simulation.  elec = 'direct' (O3) or 'fft' (O8)."""
 
-    def __init__(self, p: Problem, elec: str = "direct", K: Optional[np.ndarray] = None):
+    def __init__(self, p: Problem, elec: str = "direct", K: Optional[np.ndarray] = None,
+                 fft_workers: Optional[int] = None):
         self.p = p
         self.elec = elec
         self.K = K
+        self.fft_workers = fft_workers      # None: numpy.fft (single thread); n: scipy.fft with n host threads
         self._box_hat = None
         self.wave = None        # (amp[3], omega, phase): E_ext(t) = g.E_ext + amp sin(omega t + phase)
 
@@ -296,8 +315,8 @@ class Oracle:
         if self.elec == "direct":
             return field_direct(self.p, K, P)
         if self._box_hat is None:
-            self._box_hat = np.fft.fftn(circular_kernel(self.p, K), axes=(1, 2, 3))
-        return field_fft(self.p, K, P, self._box_hat)
+            self._box_hat = _fftn(circular_kernel(self.p, K), (1, 2, 3), self.fft_workers)
+        return field_fft(self.p, K, P, self._box_hat, self.fft_workers)
 
     def fields(self, P: np.ndarray, terms: int = TERM_ALL, t: float = 0.0):
         p = self.p
