@@ -7,7 +7,8 @@
 A step = one forward-Euler step of the whole hot path (pruned x/y transforms, fused z
 transform + tensor multiply, inverse transforms, fused local step) over the synthetic workload.  One JSON line
 is printed by rank 0.  N > 1: every rank runs an independent replica of the workload (batch sharding, no
-data-path collective), value = all ranks' cell-updates / max-over-ranks time.
+data-path collective), value = all ranks' cell-updates / max-over-ranks time.  Started
+without a torchrun environment, `--gpus N` (N > 1) re-executes itself under torch.distributed.run with N ranks.
 """
 from __future__ import annotations
 
@@ -47,11 +48,12 @@ def make_workload(name: str, dtype: str) -> fi.Workload:
 
 
 def sample_workload(name: str) -> fi.Workload:
-    """Bounded sample of the benchmark workload for the CPU oracle: same recipe (BaTiO3 300 K, 1 nm cells, open
-    boundaries, |P| = 0.26 sphere-uniform, Euler dt* = 0.002), 64x64x32 cells instead of 256x256x128."""
+    """Bounded sample of the benchmark workload for the CPU oracle: one member of config 5b
+    (128x128x64 cells, the same recipe as 5a: BaTiO3 300 K, 1 nm cells, open boundaries, |P| = 0.26 sphere-uniform,
+    Euler dt* = 0.002) instead of the 256x256x128 cells of config 5a."""
     if name == "cfg1":
         return fi.config1()
-    return fi.open_batio3("sample_64x64x32", (64, 64, 32), 1, "f64", 1005)
+    return fi.open_batio3("cfg5b_member0_128x128x64", (128, 128, 64), 1, "f64", 1005)
 
 
 def peaks():
@@ -116,11 +118,25 @@ class ClockSampler:
 
 
 # ---------------------------------------------------------------------------------------------------------
-def algorithmic_bytes(w: fi.Workload, rsz: int):
-    """Algorithmic bytes per launch of each kernel: what the pass must read and
-    write once, spectra counted with Lx = m_x/2 + 1 columns."""
+def padded_dims(w: fi.Workload):
+    """Transform length per axis: the axis itself when periodic, the power of two >= 2 n when open (A16)."""
+    m = []
+    for a in range(3):
+        if w.periodic[a]:
+            m.append(w.n[a])
+        else:
+            v = 4
+            while v < 2 * w.n[a]:
+                v *= 2
+            m.append(v)
+    return m
+
+
+def moved_bytes(w: fi.Workload, rsz: int):
+    """Bytes each kernel of the CURRENT pipeline must read and write once per launch: spectra
+    counted with Lx = m_x/2 + 1 columns, E_elec materialised between the x inverse pass and the local step."""
     nx, ny, nz = w.n
-    m = [w.n[a] if w.periodic[a] else 2 * w.n[a] for a in range(3)]
+    m = padded_dims(w)
     Lx, B, c = m[0] // 2 + 1, w.batch, 2 * rsz
     N = nx * ny * nz
     return {
@@ -131,6 +147,65 @@ def algorithmic_bytes(w: fi.Workload, rsz: int):
         "xinv": B * 3 * (N * rsz + nz * ny * Lx * c),
         "local": B * 3 * N * rsz * 3,          # read P, read E_elec, write P_new
     }
+
+
+def survey_bytes_per_cell(w: fi.Workload, rsz: int) -> float:
+    """SURVEY.md 8(d) "Algorithmic bytes per cell-RHS": per component s (1 + 4 p_x + 4 p_x p_y) with p_a = m_a / n_a,
+    tensor 6 s p_x p_y p_z / 8 shared by the B members, local step 3 s read + 3 s write (E_elec consumed on chip):
+    696 B for the open fp64 case at B = 1 (660 at B = 4, 651 at B = 16), 348 B in fp32."""
+    m = padded_dims(w)
+    px, py, pz = (m[a] / w.n[a] for a in range(3))
+    return 3 * rsz * (1 + 4 * px + 4 * px * py) + 6 * rsz * px * py * pz / 8 / w.batch + 6 * rsz
+
+
+_peaks_lib = None
+
+
+def peaks_lib():
+    """libfe_peaks.so: bench.py's own harness kernels (csrc/bench_peaks.cu); not part of the product library."""
+    global _peaks_lib
+    if _peaks_lib is None:
+        import ctypes
+        from paper_2605_28800_b200 import build as b
+        L = ctypes.CDLL(b.PEAKS_LIB)
+        vp, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double)
+        L.fe_peak_fp64.argtypes = [vp, ctypes.c_int, ctypes.c_int, dp, vp]
+        L.fe_peak_lds.argtypes = [vp, ctypes.c_int, ctypes.c_int, dp, vp]
+        L.fe_peak_l2.argtypes = [vp, vp, ctypes.c_int64, ctypes.c_int, dp, vp]
+        L.fe_bench_kmul.argtypes = [vp, vp, vp, ctypes.c_int64, ctypes.c_int, ctypes.c_int, vp]
+        _peaks_lib = L
+    return _peaks_lib
+
+
+def measure_unit_peaks(torch, dev):
+    """fp64 issue rate, shared-memory and L2 read bandwidth of THIS box, timed with CUDA events inside the harness
+    library (SURVEY.md 8(d) "Which roofline": the ALU bound is reported beside the HBM bound)."""
+    import ctypes
+    L = peaks_lib()
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    scratch = torch.zeros(148 * 8 * 256 * 4, dtype=torch.float64, device=dev)
+    out = ctypes.c_double(0.0)
+    res = {}
+    if L.fe_peak_fp64(ctypes.c_void_p(scratch.data_ptr()), 4, 4096, ctypes.byref(out), st) == 0:
+        res["fp64_warp_inst_per_s"] = out.value
+        res["fp64_tflops"] = out.value * 64 / 1e12          # one DFMA warp instruction = 32 lanes x 2 flops
+    if L.fe_peak_lds(ctypes.c_void_p(scratch.data_ptr()), 4, 4096, ctypes.byref(out), st) == 0:
+        res["lds_gbs"] = out.value / 1e9
+    buf = torch.zeros(32 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)       # 32 MB: fits L2
+    if L.fe_peak_l2(ctypes.c_void_p(buf.data_ptr()), ctypes.c_void_p(scratch.data_ptr()), buf.numel() * 8, 20,
+                    ctypes.byref(out), st) == 0:
+        res["l2_read_gbs"] = out.value / 1e9
+    return res
+
+
+def ncu_counters(workload: str, dtype: str):
+    """Per-launch counters of the committed ncu capture (profiles/ncu_traffic.json): DRAM bytes, fp64-pipe warp
+    instructions and shared-memory wavefronts per kernel."""
+    tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(tp):
+        return {}
+    with open(tp) as fh:
+        return json.load(fh).get("%s_%s" % (workload, dtype), {})
 
 
 def run_cuda(args):
@@ -167,7 +242,8 @@ def run_cuda(args):
 
     # ---- device-resident timing: W warm-up steps, then exactly K steps in one fe_step call -------------
     # warm-up: the W requested steps, then more until the GPU has been busy for ~0.5 s (a cold device ramps its clocks
-    # and power state over the first tenths of a second: the first run on a fresh box was 10 % slow without this)
+    # and power state over the first tenths of a second: the first run on a fresh box was 10 % slow without this).
+    # The JSON line prints both the requested and the executed count.
     g.step(P, w.dt, args.warmup, fe.FE_EULER, fe.FE_TERM_ALL)
     torch.cuda.synchronize()
     warm, t_w = args.warmup, time.perf_counter()
@@ -195,32 +271,60 @@ def run_cuda(args):
     g.step(P, w.dt, args.steps, fe.FE_EULER, fe.FE_TERM_ALL)
     prof = g.profile_read()
     g.profile(False)
-    alg = algorithmic_bytes(w, rsz)
+    alg = moved_bytes(w, rsz)
     pk, pk_kind = peaks()
+    hbm = pk["hbm_gbs"]
+    unit = measure_unit_peaks(torch, dev) if rank == 0 else {}
+    ctr = ncu_counters(args.workload, args.dtype)
     kern = {}
     for k, (tms, cnt) in prof.items():
         if cnt and k in alg:
             dur = tms / cnt
-            kern[k] = {"ms": dur, "alg_gbs": alg[k] / (dur * 1e-3) / 1e9, "launches": cnt}
+            row = {"ms": dur, "alg_gbs": alg[k] / (dur * 1e-3) / 1e9, "frac_hbm": alg[k] / (dur * 1e-3) / 1e9 / hbm,
+                   "launches": cnt}
+            c = ctr.get(k) if isinstance(ctr.get(k), dict) else None
+            if c and unit.get("fp64_warp_inst_per_s") and c.get("fp64_warp_inst"):
+                row["frac_fp64"] = c["fp64_warp_inst"] / (dur * 1e-3) / unit["fp64_warp_inst_per_s"]
+            if c and unit.get("lds_gbs") and c.get("smem_wavefronts"):
+                row["frac_lds"] = c["smem_wavefronts"] * 128 / (dur * 1e-3) / 1e9 / unit["lds_gbs"]
+            kern[k] = row
     prof_total = sum(v["ms"] for v in kern.values())
     dom = max(kern, key=lambda k: kern[k]["ms"])
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "ncu_traffic.json")     # bytes per launch from the committed ncu capture
-    if os.path.exists(tp):
-        with open(tp) as fh:
-            traffic = json.load(fh).get("%s_%s" % (args.workload, args.dtype), {}).get(dom)
+    cdom = ctr.get(dom) if isinstance(ctr.get(dom), dict) else {}
+    traffic = cdom.get("dram_bytes") if cdom else (ctr.get(dom) if not isinstance(ctr.get(dom), dict) else None)
     # kernel that serves the profile slot on the size-specialised path (every bench workload but cfg1 takes it)
     fast_names = {"xfwd": "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>", "xinv": "k2_xinv",
                   "local": "k_local2"}
-    generic = os.environ.get("FE_B200_GENERIC") == "1" or args.workload == "cfg1"
-    roofline = {"bound": "hbm", "kernel": ("k_" + dom) if generic else fast_names.get(dom, "k_" + dom), "achieved": kern[dom]["alg_gbs"], "peak": pk["hbm_gbs"],
+    generic = args.workload == "cfg1"
+    # which roofline binds the dominant kernel: the largest of its fractions of the three measured unit peaks
+    fr = {"hbm": kern[dom]["frac_hbm"], "alu": kern[dom].get("frac_fp64", 0.0), "lds": kern[dom].get("frac_lds", 0.0)}
+    bound = max(fr, key=lambda k: fr[k])
+    step_s = ms / args.steps * 1e-3
+    sv = survey_bytes_per_cell(w, rsz)
+    roofline = {"bound": bound, "bound_fracs": fr,
+                "kernel": ("k_" + dom) if generic else fast_names.get(dom, "k_" + dom),
+                "achieved": kern[dom]["alg_gbs"], "peak": hbm,
                 "peak_kind": pk_kind + " (burst copy bandwidth, MEASURED_PEAKS.json)", "unit": "GB/s",
-                "frac": kern[dom]["alg_gbs"] / pk["hbm_gbs"], "traffic": traffic,
+                "frac": kern[dom]["alg_gbs"] / hbm, "traffic": traffic,
                 "share_of_step": kern[dom]["ms"] / prof_total,
-                "whole_step": {"alg_bytes_per_cell": sum(alg.values()) / cells,
-                               "achieved": sum(alg.values()) / (ms / args.steps * 1e-3) / 1e9,
-                               "frac": sum(alg.values()) / (ms / args.steps * 1e-3) / 1e9 / pk["hbm_gbs"]},
-                "kernels": kern}
+                "alu": None, "lds": None,
+                "whole_step": {"alg_bytes_per_cell": sv, "alg_model": "SURVEY.md 8(d): E_elec on chip, m_x/2 columns",
+                               "moved_bytes_per_cell": sum(alg.values()) / cells,
+                               "achieved": sv * cells / step_s / 1e9,
+                               "frac": sv * cells / step_s / 1e9 / hbm,
+                               "frac_of_nominal_8000": sv * cells / step_s / 1e9 / 8000.0,
+                               "moved_frac": sum(alg.values()) / step_s / 1e9 / hbm},
+                "unit_peaks": unit, "kernels": kern}
+    if unit.get("fp64_warp_inst_per_s") and cdom.get("fp64_warp_inst"):
+        ach = cdom["fp64_warp_inst"] / (kern[dom]["ms"] * 1e-3)
+        roofline["alu"] = {"peak": unit["fp64_warp_inst_per_s"], "peak_kind": "measured (dependent DFMA chains, bench_peaks.cu)",
+                           "unit": "fp64 warp-inst/s", "achieved": ach, "frac": ach / unit["fp64_warp_inst_per_s"],
+                           "inst_per_launch": cdom["fp64_warp_inst"], "inst_source": "ncu sm__inst_executed_pipe_fp64 (profiles/ncu_traffic.json)"}
+    if unit.get("lds_gbs") and cdom.get("smem_wavefronts"):
+        ach = cdom["smem_wavefronts"] * 128 / (kern[dom]["ms"] * 1e-3) / 1e9
+        roofline["lds"] = {"peak": unit["lds_gbs"], "peak_kind": "measured (conflict-free 128-bit LDS, bench_peaks.cu)",
+                           "unit": "GB/s", "achieved": ach, "frac": ach / unit["lds_gbs"],
+                           "wavefronts_per_launch": cdom["smem_wavefronts"]}
 
     # ---- end to end through the C ABI with host buffers: every step copies its input state from pinned host memory,
     # runs one step and copies the result back to pinned host memory.  Serial: the three phases back to back.
@@ -274,7 +378,8 @@ def run_cuda(args):
             cufft = cufft_pipeline_ms(torch, w, args.dtype, dev)
             ours = sum(kern[k]["ms"] for k in ("xfwd", "yfwd", "zmul", "yinv", "xinv") if k in kern)
             cufft["ours_ms"] = ours
-            cufft["speedup"] = cufft["ms"] / ours
+            cufft["speedup"] = cufft["ms_tight"] / ours
+            cufft["speedup_vs_eager"] = cufft["ms_eager"] / ours
         except Exception as exc:      # out of memory on small boxes etc.: report, do not fail the bench
             cufft = {"error": str(exc)[:200]}
 
@@ -284,10 +389,12 @@ def run_cuda(args):
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": warm, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "warmup": warm, "warmup_requested": args.warmup_requested,
+                "warmup_note": "requested steps, then 20-step batches until the device has been busy for 0.5 s",
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
                 "config": {"workload": w.name, "grid": list(w.n), "batch": w.batch, "integrator": "euler",
-                           "terms": "landau+gradient+elec+ext", "padded_fft": [2 * v for v in w.n],
+                           "terms": "landau+gradient+elec+ext", "padded_fft": padded_dims(w),
                            "l2": "state and spectra exceed L2 (P 3N reals, spectra >= 4x that)",
                            "parallelism": "replicas x%d" % world},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
@@ -299,45 +406,73 @@ def run_cuda(args):
 
 
 def cufft_pipeline_ms(torch, w, dtype, dev):
-    """torch.fft (cuFFT) on the zero-padded box + an elementwise 6-component multiply, same sizes."""
+    """The paper's design (cuFFT + custom kernels for the intermediate operations) on the same sizes:
+    pad copy, rfftn of the padded box, 6-component multiply, irfftn, crop.  Timed twice: `tight` = padded box, spectrum
+    and output preallocated, plans warm, the multiply one fused harness kernel (bench_peaks.cu: fe_bench_kmul), the crop a
+    view; `eager` = the same written with eager tensor arithmetic and fresh allocations (round 1's figure)."""
+    import ctypes
     td = torch.float64 if dtype == "f64" else torch.float32
     nx, ny, nz = w.n
-    m = [w.n[a] if w.periodic[a] else 2 * w.n[a] for a in range(3)]
+    m = padded_dims(w)
     B = w.batch
+    hx = m[0] // 2 + 1
     P = torch.randn(B, 3, nz, ny, nx, device=dev, dtype=td)
-    K = [torch.randn(m[2], m[1], m[0] // 2 + 1, device=dev, dtype=td) for _ in range(6)]
+    K6 = torch.randn(6, m[2], m[1], hx, device=dev, dtype=td)
     idx = ((0, 3, 4), (3, 1, 5), (4, 5, 2))
+    L = peaks_lib()
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
 
-    def once():
-        Pp = torch.zeros(B, 3, m[2], m[1], m[0], device=dev, dtype=td)
-        Pp[:, :, :nz, :ny, :nx] = P
+    Pp = torch.zeros(B, 3, m[2], m[1], m[0], device=dev, dtype=td)          # padding zeroed once: only the corner changes
+    nk = m[2] * m[1] * hx
+
+    def tight():
+        Pp[:, :, :nz, :ny, :nx].copy_(P)
         Ph = torch.fft.rfftn(Pp, dim=(2, 3, 4))
-        del Pp
-        Eh = torch.stack([sum(K[idx[i][j]] * Ph[:, j] for j in range(3)) for i in range(3)], dim=1)
+        Eh = torch.empty_like(Ph)
+        if L.fe_bench_kmul(ctypes.c_void_p(Ph.data_ptr()), ctypes.c_void_p(K6.data_ptr()), ctypes.c_void_p(Eh.data_ptr()),
+                           nk, B, 0 if dtype == "f64" else 1, st) != 0:
+            raise RuntimeError("fe_bench_kmul failed")
+        del Ph
+        return torch.fft.irfftn(Eh, s=(m[2], m[1], m[0]), dim=(2, 3, 4))[:, :, :nz, :ny, :nx]
+
+    def eager():
+        Pq = torch.zeros(B, 3, m[2], m[1], m[0], device=dev, dtype=td)
+        Pq[:, :, :nz, :ny, :nx] = P
+        Ph = torch.fft.rfftn(Pq, dim=(2, 3, 4))
+        del Pq
+        Eh = torch.stack([sum(K6[idx[i][j]] * Ph[:, j] for j in range(3)) for i in range(3)], dim=1)
         del Ph
         return torch.fft.irfftn(Eh, s=(m[2], m[1], m[0]), dim=(2, 3, 4))[:, :, :nz, :ny, :nx].contiguous()
 
-    for _ in range(2):
-        once()
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps = 3
-    e0.record()
-    for _ in range(reps):
-        once()
-    e1.record()
-    torch.cuda.synchronize()
-    return {"ms": e0.elapsed_time(e1) / reps, "what": "torch.fft.rfftn/irfftn (cuFFT) on the padded box + multiply"}
+    def timeit(fn, reps):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    t_tight = timeit(tight, 5)
+    t_eager = timeit(eager, 3)
+    return {"ms": t_tight, "ms_tight": t_tight, "ms_eager": t_eager,
+            "what": "torch.fft.rfftn/irfftn (cuFFT) on the padded box; tight = preallocated padded box (zeroed once), warm "
+                    "plans, one fused multiply kernel, crop as a view; eager = fresh allocations and eager tensor arithmetic"}
 
 
 # ---------------------------------------------------------------------------------------------------------
-def oracle_steps(workload: str, steps: int, warmup: int):
-    """Time the CPU oracle as it stands (oracle-FFT electrostatics O8 + Landau + gradient + Euler) on the sample."""
+def oracle_steps(workload: str, steps: int, warmup: int, threads: int):
+    """Time the CPU oracle as it stands (oracle-FFT electrostatics O8 + Landau + gradient + Euler) on the sample.
+    threads = 1: numpy.fft and one OpenMP thread; threads > 1: scipy.fft workers and that many OpenMP threads."""
+    os.environ["OMP_NUM_THREADS"] = str(threads)
     from oracle import fe_oracle as orc
     w = sample_workload(workload)
     p = orc.Problem(n=w.n, d=w.d, periodic=w.periodic, pbc_images=w.pbc_images, materials=w.materials[0],
                     g=w.globals_[0], matmap=w.matmap)
-    o = orc.Oracle(p, elec="fft")
+    o = orc.Oracle(p, elec="fft", fft_workers=threads if threads > 1 else None)
     o.table()                                  # tensor table: once per geometry, outside the timed region
     P = w.P0[0].copy()
     for _ in range(warmup):
@@ -349,12 +484,22 @@ def oracle_steps(workload: str, steps: int, warmup: int):
     return w, dt
 
 
+def host_threads() -> int:
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:
+        return max(1, os.cpu_count() or 1)
+
+
 def cpu_baseline(workload: str):
-    w, dt = oracle_steps(workload, 3, 1)
-    return {"value": w.cells * 3 / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "%s: %dx%dx%d cells of the same recipe, 3 Euler steps, oracle-FFT electrostatics (numpy.fft) + "
-                      "C loops for Landau/gradient, single thread; tensor table built outside the timed region"
-                      % (w.name, *w.n), "host_cores": os.cpu_count()}
+    """the oracle on all host cores of the box (OpenMP loops + threaded library FFT), on one
+    member of config 5b, 3 Euler steps after 1 warm-up step; tensor table outside the timed region."""
+    th = host_threads()
+    w, dt = oracle_steps(workload, 3, 1, th)
+    return {"value": w.cells * 3 / dt, "unit": UNIT, "cores": th, "kind": "oracle",
+            "sample": "%s: %dx%dx%d cells of the same recipe, 3 Euler steps, oracle-FFT electrostatics (scipy.fft, %d workers) "
+                      "+ OpenMP C loops for Landau / gradient; tensor table built outside the timed region"
+                      % (w.name, *w.n, th), "host_cores": os.cpu_count()}
 
 
 def run_reference(args):
@@ -363,14 +508,15 @@ def run_reference(args):
         return
     steps, warm = args.steps, min(args.warmup, 1)
     steps = min(steps, 10)
-    w, dt = oracle_steps(args.workload, steps, warm)
+    th = host_threads()
+    w, dt = oracle_steps(args.workload, steps, warm, th)
     value = w.cells * steps / dt
-    sample = "%s (%dx%dx%d cells, same recipe as %s), %d Euler steps" % (w.name, *w.n, args.workload, steps)
+    sample = "%s (%dx%dx%d cells, same recipe as %s), %d Euler steps, %d host threads" % (w.name, *w.n, args.workload, steps, th)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
             "steps": steps, "warmup": warm, "ms_per_step": dt / steps * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": make_workload_name(args.workload), "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": th, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
@@ -378,6 +524,22 @@ def run_reference(args):
 def make_workload_name(name: str) -> str:
     return {"cfg5a": "cfg5a_256x256x128", "cfg5b": "cfg5b_128x128x64_b4", "cfg3": "cfg3_sweep_64^3_b16",
             "cfg1": "cfg1_tiny_16x16x8"}[name]
+
+
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` outside torchrun: start N ranks (one per GPU) of this same script under
+    torch.distributed.run, rendezvous on 127.0.0.1, and pass the exit code on."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit("bench.py --gpus %d: only %d CUDA device(s) visible" % (args.gpus, have))
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -391,10 +553,15 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison leg")
     args = ap.parse_args()
+    args.warmup_requested = args.warmup
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
     else:
+        if args.gpus != int(os.environ.get("WORLD_SIZE", "1")):
+            raise SystemExit("bench.py: --gpus %d does not match WORLD_SIZE=%s" % (args.gpus, os.environ.get("WORLD_SIZE")))
         run_cuda(args)
 
 

@@ -42,7 +42,7 @@ typedef enum {
     FE_ENOMEM = 2,      /* workspace too small / allocation of the small tables failed               */
     FE_ECUDA = 3,       /* a CUDA call failed; text in fe_last_error()                              */
     FE_ESTATE = 4,      /* call order: no workspace bound, tensor not precomputed, material unset    */
-    FE_ENONFINITE = 5   /* fe_energy found NaN/Inf                                                  */
+    FE_ENONFINITE = 5   /* fe_energy found NaN/Inf; fe_step_rk45: error estimate NaN/Inf 8 attempts in a row */
 } fe_status;
 
 enum { FE_F64 = 0, FE_F32 = 1 };
@@ -92,8 +92,6 @@ fe_status fe_bind_workspace(fe_grid* g, void* dev, size_t bytes);
 fe_status fe_set_material(fe_grid* g, int32_t member, int32_t material_id, const fe_landau* m);
 fe_status fe_set_global(fe_grid* g, int32_t member, const fe_global* gl);
 fe_status fe_set_external_field(fe_grid* g, int32_t member, const double E[3]);
-/* dev_map: uint8 [nz][ny][nx] material id per cell, shared by the batch; NULL = all cells material 0.
- * Borrowed (not copied). */
 /* Time-dependent external excitation: E_ext(t) = E (fe_set_external_field) + amp sin(omega t + phase),
  * sampled at the stage times of the integrator (t_n, t_n + dt/2, ... ; c_i h for RK45).  amp = 0 switches it off.
  * The grid keeps a clock: fe_step / fe_step_rk45 advance it, fe_rhs and fe_energy sample E_ext at it. */
@@ -102,6 +100,8 @@ fe_status fe_set_external_wave(fe_grid* g, int32_t member /* -1 = all */, const 
 fe_status fe_set_time(fe_grid* g, double t);
 fe_status fe_get_time(const fe_grid* g, double* t);
 
+/* dev_map: DEVICE uint8 [nz][ny][nx] material id per cell (every id < n_materials), shared by the batch;
+ * NULL = all cells material 0.  Borrowed (not copied) until the next call or fe_destroy_grid.  PAPER.md:117. */
 fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map);
 
 /* a0: cell-averaged dipolar tensor K_ij(d) on the padded box and its real spectrum (once per
@@ -121,7 +121,8 @@ fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int32_t integr
  * |y5 - y4| / tol (tol: absolute, in the units of P); a step is accepted when err <= 1, then
  * dt_next = 0.9 dt err^-0.2 (5 dt when err <= 1.89e-4), else dt = max(0.9 dt err^-0.25, 0.1 dt) and the step is
  * retried; the last step is shortened to land on t_span.  All batch members advance with the same step.  At most
- * max_steps attempts are made (stats->t < t_span then).  Synchronises the stream once per attempt (the decision
+ * max_steps attempts are made (stats->t < t_span then).  A NaN / Inf error estimate rejects the attempt; after 8
+ * such attempts in a row the call returns FE_ENONFINITE (P holds the last accepted state).  Synchronises the stream once per attempt (the decision
  * is taken on the host); *stats is HOST memory and may be NULL.  Needs the workspace of fe_workspace_bytes. */
 typedef struct {
     double t;            /* time reached */

@@ -255,7 +255,7 @@ class Grid:
             raise RuntimeError("paper_2605_28800_b200 needs a CUDA device (no CPU path exists)")
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
-        self.n, self.batch = tuple(int(v) for v in n), int(batch)
+        self.n, self.batch, self.n_materials = tuple(int(v) for v in n), int(batch), int(n_materials)
         self.tdtype = torch.float64 if dtype == "f64" else torch.float32
         self.h = fe_create_grid(n, d, periodic, pbc_images, batch, FE_F64 if dtype == "f64" else FE_F32,
                                 n_materials, zero_mode)
@@ -290,24 +290,42 @@ class Grid:
     def time(self) -> float: return fe_get_time(self.h)
 
     def set_material_map(self, dev_map: Optional[torch.Tensor]):
+        if dev_map is not None:
+            nx, ny, nz = self.n
+            if not (dev_map.is_cuda and dev_map.device == self.device and dev_map.dtype == torch.uint8
+                    and dev_map.is_contiguous() and tuple(dev_map.shape) == (nz, ny, nx)):
+                raise FeError(FE_EINVAL, "material map must be a contiguous uint8 [nz][ny][nx] tensor on %s" % self.device)
+            if int(dev_map.max()) >= self.n_materials:
+                raise FeError(FE_EINVAL, "material map holds an id >= n_materials = %d" % self.n_materials)
         self._map = dev_map          # keep the borrowed tensor alive
         fe_set_material_map(self.h, dev_map)
+
+    def _state_ok(self, P: torch.Tensor, what: str = "P"):
+        """The kernels trust the pointer: refuse anything that is not the ABI's [B][3][nz][ny][nx] array."""
+        if not (isinstance(P, torch.Tensor) and P.is_cuda and P.device == self.device and P.dtype == self.tdtype
+                and P.is_contiguous() and tuple(P.shape) == self.state_shape):
+            raise FeError(FE_EINVAL, "%s must be a contiguous %s tensor of shape %s on %s"
+                          % (what, self.tdtype, self.state_shape, self.device))
 
     def precompute_tensor(self): fe_precompute_tensor(self.h)
 
     def rhs(self, P: torch.Tensor, terms=FE_TERM_ALL) -> torch.Tensor:
+        self._state_ok(P)
         out = torch.empty_like(P)
         fe_rhs(self.h, P, out, terms)
         return out
 
     def step(self, P: torch.Tensor, dt, nsteps, integrator=FE_EULER, terms=FE_TERM_ALL):
+        self._state_ok(P)
         fe_step(self.h, P, dt, nsteps, integrator, terms)
         return P
 
     def step_rk45(self, P: torch.Tensor, t_span, dt_init, tol, max_steps=100000, terms=FE_TERM_ALL) -> dict:
+        self._state_ok(P)
         return fe_step_rk45(self.h, P, t_span, dt_init, tol, max_steps, terms)
 
     def energy(self, P: torch.Tensor, terms=FE_TERM_ALL, allow_nonfinite=False) -> np.ndarray:
+        self._state_ok(P)
         return fe_energy(self.h, P, self.batch, terms, allow_nonfinite)
 
     def get_tensor(self) -> np.ndarray: return fe_get_tensor(self.h)

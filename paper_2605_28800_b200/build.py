@@ -16,6 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libfe_b200.so")
+PEAKS_LIB = os.path.join(HERE, "libfe_peaks.so")      # bench.py's harness kernels (csrc/bench_peaks.cu), not the product
 SOURCES = ["fe_api.cu", "fe_fft.cu", "fe_fft2_x.cu", "fe_fft2_axis.cu", "fe_fft2_z.cu", "fe_tensor.cu", "fe_local.cu", "fe_integ.cu"]
 HEADERS = [os.path.join(CSRC, "fe_internal.h"), os.path.join(CSRC, "fe_fft2.cuh"), os.path.join(ROOT, "include", "fe.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -54,6 +55,9 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
                     print(out)
     if jobs or not os.path.exists(LIB):
         run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs])
+    peaks_src = os.path.join(CSRC, "bench_peaks.cu")
+    if force or _stale(PEAKS_LIB, [peaks_src]):
+        run([NVCC, *FLAGS, "-shared", peaks_src, "-o", PEAKS_LIB])
     return LIB
 
 

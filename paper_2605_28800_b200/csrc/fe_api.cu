@@ -225,21 +225,18 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     q.pitch = (q.Lx + pl - 1) / pl * pl;
     q.pitch64 = (q.Lx + 7) / 8 * 8;
     {
-        // FE_B200_GENERIC=1 forces the generic shared-memory passes (debugging aid; both paths are tested)
-        const char* env = getenv("FE_B200_GENERIC");
-        const bool generic = env && env[0] == '1';
+        // size-specialised register passes per axis; any other transform length takes the generic shared-memory pass
         const size_t lanes_full = 128 / g->csz;
-        g->fast[0] = !generic && x2_supported(q.m[0] / 2);
-        g->fast[1] = !generic && axis2_supported(q.m[1]) && (size_t)q.lanes == lanes_full;
-        g->fast[2] = !generic && zmul2_supported(q.m[2]) && (size_t)q.lanes == lanes_full;
+        g->fast[0] = x2_supported(q.m[0] / 2);
+        g->fast[1] = axis2_supported(q.m[1]) && (size_t)q.lanes == lanes_full;
+        g->fast[2] = zmul2_supported(q.m[2]) && (size_t)q.lanes == lanes_full;
         // Tiled layouts (L = 128 bytes of consecutive kx, G = pitch / L groups), used when every pass is fast:
         //   S1[b][c][z][g][y][L]   the y pass reads / writes whole contiguous tiles,
         //   S2[b][c][g][z][ky][L]  likewise (ky in slot order when the bulk-copy y pass runs); the fused z pass reads
         //                          128-byte rows 64 KB apart instead of 2 MB apart,
         //   Kt[6][g][ky][kz][L]    its tensor tile is contiguous too.
-        // FE_B200_LINEAR=1 keeps the row-major layouts (tuning aid).
-        const char* lin = getenv("FE_B200_LINEAR");
-        g->tiled = g->fast[0] && g->fast[1] && g->fast[2] && !(lin && lin[0] == '1');
+        // otherwise the spectra stay row-major (the kernels take strides, both layouts run the same code).
+        g->tiled = g->fast[0] && g->fast[1] && g->fast[2];
     }
     g->dirty = true;
     g->mixed = 0;
@@ -563,9 +560,8 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     const int64_t y2_sa = tl ? L : p, y2_sg = tl ? (int64_t)My * nz * L : L, y2_sz = tl ? (int64_t)My * L : p * My,
                   y2_sb = p * My * nz;                                                          // S2, y pass
     const int64_t zs[4] = {p * My * nz, tl ? (int64_t)My * L : p * My, tl ? L : p, tl ? (int64_t)My * nz * L : L};
-    // bulk-copy y pass (contiguous tiles, ky of S2 in slot order); FE_B200_Y4=0 falls back to the register-I/O pass
-    static const bool y4off = getenv("FE_B200_Y4") && getenv("FE_B200_Y4")[0] == '0';
-    const bool use4 = tl && !y4off && axis4_supported(My);
+    // bulk-copy y pass (contiguous tiles, ky of S2 in slot order) for the long axes; register-I/O pass otherwise
+    const bool use4 = tl && axis4_supported(My);
     int perm[3] = {0, 0, 0};
     if (use4) axis4_radices(My, perm);
     const int64_t ks[4] = {(int64_t)Hz * Hy * p, tl ? L : (int64_t)Hy * p, tl ? (int64_t)Hz * L : p,
@@ -760,8 +756,7 @@ extern "C" fe_status fe_step(fe_grid* g, void* P, double dt, int32_t nsteps, int
     // on an internal stream ordered with the caller's stream by events: small grids are launch bound otherwise.
     // The first unit always runs eagerly (one-time kernel attribute set-up must not happen inside a capture).
     const int unit = integ == FE_EULER ? 2 : 1;
-    static const bool graphs_off = getenv("FE_B200_GRAPH") && getenv("FE_B200_GRAPH")[0] == '0';
-    if (g->prof_on || g->goff || graphs_off || nsteps < 6 * unit || integ == FE_AB3M2 || g->any_wave) {
+    if (g->prof_on || g->goff || nsteps < 6 * unit || integ == FE_AB3M2 || g->any_wave) {
         s = run(nsteps, st);             // (a time-dependent E_ext changes the kernel arguments from step to step)
         if (s == FE_OK) g->time = time0 + nsteps * dt;
         mark(g, -1, st);
@@ -836,7 +831,7 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
     const size_t bytes = (size_t)n * sizeof(T);
     const double time0 = g->time;
     double t = 0.0, dt = dt_init, err = 0.0, dt_last = 0.0;
-    int acc = 0, rej = 0, evals = 0;
+    int acc = 0, rej = 0, evals = 0, nonfinite = 0;
     fe_status s;
     while (t < t_span && acc + rej < max_steps) {
         const double h = dt < t_span - t ? dt : t_span - t;
@@ -866,13 +861,20 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
         err = emax / tol;
         if (err <= 1.0) {                                // NaN compares false: a non-finite estimate rejects
             FE_CUDA(cudaMemcpyAsync(P, Y5, bytes, cudaMemcpyDeviceToDevice, st));
-            t += h; ++acc; dt_last = h;
+            t += h; ++acc; dt_last = h; nonfinite = 0;
             dt = err <= 1.89e-4 ? 5.0 * h : 0.9 * h * pow(err, -0.2);
         } else {
             ++rej;
             const double shr = 0.9 * h * pow(err, -0.25);
             dt = (shr > 0.1 * h) ? shr : 0.1 * h;         // also taken when err is NaN
-            if (!isfinite(err) && rej > 60) return fail(FE_ENONFINITE, "RK45: non-finite error estimate");
+            // a stage that overflowed may recover with a smaller step; a state that already holds NaN / Inf never does
+            if (isfinite(err)) nonfinite = 0;
+            else if (++nonfinite >= 8) {
+                g->time = time0 + t;
+                if (out) { out->t = t; out->dt_last = dt_last; out->dt_next = dt; out->err_last = err;
+                           out->accepted = acc; out->rejected = rej; out->rhs_evals = evals; }
+                return fail(FE_ENONFINITE, "RK45: non-finite error estimate in 8 consecutive attempts");
+            }
         }
     }
     FE_CUDA(cudaStreamSynchronize(st));

@@ -201,19 +201,15 @@ static cudaError_t launch_one(const void* in, void* out, const X2Args& a, cudaSt
 {
     using C = XCfg<M>;
     constexpr size_t smem = (size_t)(2 * M + C::ROWS * C::RPITCH) * sizeof(cx<T>);
-    static bool configured = false;
     const dim3 grid((unsigned)((a.nrows + C::ROWS - 1) / C::ROWS));
     if constexpr (FWD) {
-        if (!configured) {
+        // persistent: as many blocks as fit on the device (rows are visited with a grid stride)
+        static PerDevice<int> cache;
+        int& nblocks = cache.here();
+        if (!nblocks) {
             cudaError_t e = cudaFuncSetAttribute(k2_xfwd<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
-            configured = true;
-        }
-        // persistent: as many blocks as fit on the device (rows are visited with a grid stride)
-        static int nblocks = 0;
-        if (!nblocks) {
             int dev = 0, sms = 0, per = 0;
-            cudaError_t e;
             if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
             if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
             if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k2_xfwd<T, M, PRUNE>, 256, smem)) != cudaSuccess) return e;
@@ -222,10 +218,12 @@ static cudaError_t launch_one(const void* in, void* out, const X2Args& a, cudaSt
         const dim3 pgrid(grid.x < (unsigned)nblocks ? grid.x : (unsigned)nblocks);
         k2_xfwd<T, M, PRUNE><<<pgrid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
     } else {
+        static PerDevice<int> cache;
+        int& configured = cache.here();
         if (!configured) {
             cudaError_t e = cudaFuncSetAttribute(k2_xinv<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
-            configured = true;
+            configured = 1;
         }
         k2_xinv<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<const cx<T>*>(in), static_cast<T*>(out), a);
     }

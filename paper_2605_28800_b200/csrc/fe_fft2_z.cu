@@ -15,7 +15,6 @@
 // Both inter-step twiddles w_M^{+-n2 k1} are applied by the thread that owns k1: it loads its R2 - 1 factors once
 // per tile and uses them for the three components in both directions (the R1-point steps move no twiddles).
 #include "fe_fft2.cuh"
-#include <stdlib.h>
 
 namespace fe {
 namespace v2 {
@@ -39,8 +38,6 @@ struct Z2Args {
     int64_t kcs, k_skz, k_sky, k_sg;
     int la, lb, lc;   // ky is stored in slot order (k1 pb + k2) pc + k3, ky = k1 + pa k2 + pa pb k3, with the binary
                       // logarithms of pa, pb, pc given; la < 0: natural order
-    int gs;           // tiles per stored group of kx (1; 2 when a tile is half a 128-byte row): tile group kxg sits at
-                      // (kxg / gs) * s_g + (kxg % gs) * LANES (gs is 1 or 2)
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
@@ -140,8 +137,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         if (a.la >= 0)
             slot = ((ky & ((1 << a.la) - 1)) << (a.lb + a.lc)) | (((ky >> a.la) & ((1 << a.lb) - 1)) << a.lc) |
                    (ky >> (a.la + a.lb));
-        return S + (int64_t)it.b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)(it.kxg >> (a.gs - 1)) * a.s_g +
-               (it.kxg & (a.gs - 1)) * LANES;
+        return S + (int64_t)it.b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)it.kxg * a.s_g;
     };
     // asynchronous copies: input rows of a tile, K~ tile of an item
     auto prefetch_tile = [&](const cx<T>* tb) {
@@ -172,8 +168,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         const int tid = (int)threadIdx.x - T0;
         const int q = tid % OPS_ROW, row0 = tid / OPS_ROW;
         const int64_t krs = a.k_skz;                                    // stride of kz in the table
-        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)(it.kxg >> (a.gs - 1)) * a.k_sg + (it.kxg & (a.gs - 1)) * LANES +
-                     (int64_t)row0 * krs + q * PER;
+        const T* g = Kt + (int64_t)it.kyh * a.k_sky + (int64_t)it.kxg * a.k_sg + (int64_t)row0 * krs + q * PER;
         T* s = kbuf + row0 * LANES + q * PER;
 #pragma unroll
         for (int c6 = 0; c6 < 6; ++c6) {
@@ -333,7 +328,8 @@ template <typename T, int M, int LANES, bool PRUNE>
 static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
 {
     using C = ZCfg<T, M, LANES, PRUNE>;
-    static int nblocks = 0;
+    static PerDevice<int> cache;
+    int& nblocks = cache.here();
     if (!nblocks) {
         cudaError_t e = cudaFuncSetAttribute(k2_zmul<T, M, LANES, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)C::smem);
@@ -347,7 +343,6 @@ static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
         nblocks = sms * (per > 0 ? per : 1);
     }
     a.nitems = a.ngroups * (a.My / 2 + 1);
-    if (a.gs != 1 && a.gs != 2) return cudaErrorInvalidValue;
     const int grid = a.nitems < nblocks ? a.nitems : nblocks;
     k2_zmul<T, M, LANES, PRUNE><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a);
     return cudaGetLastError();
@@ -380,23 +375,14 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
         }
     }
     v2::Z2Args a{c.tw, members, My, batch, nz, ngroups, 0, sstr[0], sstr[1], sstr[2], sstr[3],
-                 kstr[0], kstr[1], kstr[2], kstr[3], lg[0], lg[1], lg[2], 1};
+                 kstr[0], kstr[1], kstr[2], kstr[3], lg[0], lg[1], lg[2]};
     const bool prune = 2 * nz <= M;              // zero-padded axis
     if (!prune && nz != M) return cudaErrorInvalidValue;
     switch (M) {
         case 64: return v2::launch_p<T, 64, L128>(prune, S, Kt, a, st);
         case 128: return v2::launch_p<T, 128, L128>(prune, S, Kt, a, st);
-        case 256: {
-            // 128-byte rows (one 256-thread block per SM) beat 64-byte rows (two 128-thread blocks) on B200:
-            // 0.66 vs 0.80 ms at cfg5a.  FE_B200_ZLANES=4 selects the narrow tile (tuning aid).
-            static const int zl = getenv("FE_B200_ZLANES") ? atoi(getenv("FE_B200_ZLANES")) : 0;
-            if (zl == 4) {
-                // half-width tiles: twice the groups, two tiles per stored group
-                a.ngroups *= 2; a.gs = 2;
-                return v2::launch_p<T, 256, L128 / 2>(prune, S, Kt, a, st);
-            }
-            return v2::launch_p<T, 256, L128>(prune, S, Kt, a, st);
-        }
+        // 128-byte rows (one 256-thread block per SM) beat 64-byte rows (two 128-thread blocks): 0.66 vs 0.80 ms at cfg5a
+        case 256: return v2::launch_p<T, 256, L128>(prune, S, Kt, a, st);
         default: return cudaErrorInvalidValue;
     }
 }

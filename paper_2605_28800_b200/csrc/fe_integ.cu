@@ -7,7 +7,7 @@
 namespace fe {
 
 template <typename T, int NK>
-__global__ void __launch_bounds__(256) k_lincomb(T* __restrict__ out, const T* __restrict__ base, LinArgs a, int64_t n)
+__global__ void __launch_bounds__(256) k_lincomb(T* out, const T* base, LinArgs a, int64_t n)   // out may alias base
 {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
         T v = base[i];
@@ -16,6 +16,9 @@ __global__ void __launch_bounds__(256) k_lincomb(T* __restrict__ out, const T* _
         out[i] = v;
     }
 }
+
+// max that keeps a NaN once it has seen one (fmax would return the other operand and hide a blown-up cell)
+__device__ __forceinline__ double nanmax(double m, double v) { return (v > m || v != v) ? v : m; }
 
 template <typename T>
 __global__ void __launch_bounds__(256) k_rk45_final(T* __restrict__ y5, const T* __restrict__ P, LinArgs b5, LinArgs d,
@@ -31,17 +34,17 @@ __global__ void __launch_bounds__(256) k_rk45_final(T* __restrict__ y5, const T*
             e = e + (T)d.c[j] * kj;
         }
         y5[i] = v;
-        m = fmax(m, fabs((double)e));
+        m = nanmax(m, fabs((double)e));
     }
-    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+    for (int o = 16; o > 0; o >>= 1) m = nanmax(m, __shfl_down_sync(0xffffffffu, m, o));
     __shared__ double red[8];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (lane == 0) red[warp] = m;
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = fmax(m, red[w]);
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) m = nanmax(m, red[w]);
         // non-negative doubles order like their bit patterns; NaN (all-ones exponent, non-zero mantissa) sorts above
-        // +inf, so a non-finite error estimate always rejects the step
+        // +inf, so a non-finite error estimate reaches the host and rejects the step
         atomicMax(err_bits, (unsigned long long)__double_as_longlong(m));
     }
 }

@@ -11,6 +11,20 @@ constexpr int kTwiddleN = 2048;      // twiddle table w[k] = exp(-2 pi i k / 204
 constexpr int kMaxStages = 6;
 constexpr int kThreads = 256;
 
+// One-time kernel set-up (dynamic shared-memory limit, persistent grid size) is a property of the DEVICE, not of the
+// process: the launchers cache it per device in a zero-initialised static PerDevice<int>.  Concurrent first calls
+// repeat the same idempotent set-up and store the same value.
+constexpr int kMaxDevices = 64;
+template <typename V> struct PerDevice {
+    V v[kMaxDevices];
+    V& here()
+    {
+        int d = 0;
+        if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= kMaxDevices) d = 0;
+        return v[d];
+    }
+};
+
 // Radix plan of one in-place power-of-two FFT of length M (complex points).
 // Forward = decimation in frequency (natural in, digit-reversed out),
 // inverse = decimation in time with the stages mirrored (digit-reversed in, natural out).

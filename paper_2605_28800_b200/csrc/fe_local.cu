@@ -7,7 +7,6 @@
 //            zero outside the sample / in vacuum cells, c_ia = G11 (a == i) or G44 + G44', Gm = G12 + G44 - G44'
 //   then the integrator stage:  Yout = baseY + cy * k,  accOut = accIn + ca * k
 #include "fe_internal.h"
-#include <stdlib.h>
 
 namespace fe {
 
@@ -641,13 +640,13 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     // z chunk: as long as possible (halo planes are re-read per chunk) while the grid still fills the machine
     int zc = a.n[2];
     while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
-    if (getenv("FE_B200_ZC")) zc = atoi(getenv("FE_B200_ZC"));   // tuning aid
     a.zchunk = zc;
     dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
     const int ns = a.map ? 4 : 5;         // ring slots of k_local2
     const size_t smem = two ? (size_t)ns * 3 * k2Tile * sizeof(T) + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1)
                             : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
-    static bool configured = false;
+    static PerDevice<int> cache;
+    int& configured = cache.here();
     if (!configured) {
         const int lim = 96 * 1024;      // 255 materials need 61 KB
         cudaError_t e = cudaFuncSetAttribute(k_local<T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim);
@@ -660,7 +659,7 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured = 1;
     }
     if (two) {
         if (a.map) {

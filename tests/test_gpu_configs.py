@@ -1,5 +1,5 @@
 """-m gpu parity tests at the FULL sizes of BASELINE.json configs 2, 3 and 4 (config 1 is tests/test_gpu_parity.py,
-config 5 the sampled full-size check of tests/test_gpu_fastpath.py), through the C ABI against the CPU oracle.
+config 5 at the end of this file: the dense seeded state, full field), through the C ABI against the CPU oracle.
 Tolerances: rel-L2 <= 1e-10 per RHS, <= 1e-8 after 100 steps (fp64).  Long relaxations are compared on observables
 (wall plateau and width against the paper's Eq. 10 values in tests/golden/wall_180_paper.txt), never cell-wise
 (reading A15)."""
@@ -146,4 +146,80 @@ def test_paper_bilayer_geometry_128x128x36(fe):
     assert np.all(got[:, w.matmap == 2] == 0.0)                   # vacuum layer
     g.step(P, w.dt, 3, fi.EULER, fi.TERM_ALL)
     assert rel_l2(P.cpu().numpy()[0], o.step(w.P0[0], w.dt, 3, fi.EULER, fi.TERM_ALL)) < 1e-10
+    g.close()
+
+
+# ---- config 5: the seeded DENSE state bench.py times, full field, at full size ----------------------------------------
+_cfg5_oracles = {}
+
+
+def _cfg5_oracle(cfg):
+    """Oracle-FFT (O8) of config 5a / 5b: the __float128 table and the transformed kernel box are built once per geometry
+    and shared by the fp64 and fp32 cases (the members of 5b share geometry and coefficients)."""
+    if cfg not in _cfg5_oracles:
+        _cfg5_oracles.clear()                                  # one geometry at a time: the 5a box spectrum is 6.4 GB
+        w = fi.config5a() if cfg == "5a" else fi.config5b()
+        o = orc.Oracle(oracle_problem(w, 0), elec="fft")
+        o._box_hat = np.fft.fftn(orc.circular_kernel(o.p, o.table()), axes=(1, 2, 3))
+        _cfg5_oracles[cfg] = (w, o)
+    return _cfg5_oracles[cfg]
+
+
+@pytest.mark.parametrize("cfg,dtype", [("5b", "f64"), ("5b", "f32"), ("5a", "f64"), ("5a", "f32")])
+def test_config5_full_field_parity(fe, cfg, dtype):
+    """Configs 5a (256x256x128, B = 1) and 5b (128x128x64, B = 4, last member) from the seeded dense state of the config,
+    in the launch configuration bench.py times: fe_rhs with TERM_ELEC and TERM_ALL against oracle-FFT over the FULL field
+    (rel-L2 <= 1e-10 fp64, <= 1e-4 fp32 against the fp64 oracle on the fp32-rounded input), six sampled cells against the
+    direct sum, Euler steps <= 1e-8 with F_tot decreasing and equal to the oracle's."""
+    w, o = _cfg5_oracle(cfg)
+    b = w.batch - 1
+    tol = 1e-10 if dtype == "f64" else 1e-4
+    P0 = w.P0 if dtype == "f64" else w.P0.astype(np.float32).astype(np.float64)
+    g = fe.Grid.from_workload(w, dtype=dtype)
+    g.precompute_tensor()
+    P = g.state(P0)
+    L = w.globals_[b].L
+    El, Eg, Ee, Ex = o.fields(P0[b], fi.TERM_ALL)
+    got = g.rhs(P, fi.TERM_ELEC)[b].cpu().numpy().astype(np.float64)
+    assert rel_l2(got, L * Ee) < tol
+    # sampled cells against the direct sum over all source cells (not the FFT)
+    t = np.random.default_rng(5).integers(0, w.cells, size=6)
+    Ed = orc.field_direct(o.p, o.table(), P0[b], targets=t)
+    assert np.max(np.abs(got.reshape(3, -1)[:, t] / L - Ed)) < tol * np.max(np.abs(Ed))
+    got = g.rhs(P, fi.TERM_ALL)[b].cpu().numpy().astype(np.float64)
+    assert rel_l2(got, L * (El + Eg + Ee + Ex)) < tol
+    del El, Eg, Ee, Ex, got
+    if dtype == "f32":
+        g.close()
+        return
+    # Euler steps from the dense state (10 at 5b, 3 at 5a: every oracle step is a 512 x 512 x 256 complex convolution)
+    nsteps = 10 if cfg == "5b" else 3
+    F = [g.energy(P)[b][4]]
+    for _ in range(nsteps):
+        g.step(P, w.dt, 1, fi.EULER, fi.TERM_ALL)
+        F.append(g.energy(P)[b][4])
+    assert all(F[i + 1] < F[i] for i in range(nsteps)) and np.isfinite(F).all()
+    ref = o.step(P0[b], w.dt, nsteps, fi.EULER, fi.TERM_ALL)
+    assert rel_l2(P[b].cpu().numpy(), ref) < 1e-8
+    assert F[-1] == pytest.approx(o.energy(ref)[4], rel=1e-9)
+    if w.batch > 1:                                            # members are independent: member 0 ran its own problem
+        ref0 = o.step(P0[0], w.dt, 1, fi.EULER, fi.TERM_ALL)
+        P1 = g.state(P0)
+        g.step(P1, w.dt, 1, fi.EULER, fi.TERM_ALL)
+        assert rel_l2(P1[0].cpu().numpy(), ref0) < 1e-10
+    g.close()
+
+
+@pytest.mark.skipif(__import__("os").environ.get("FE_TEST_SLOW") != "1",
+                    reason="the oracle's __float128 table at R = 10 takes ~10 min of host time: FE_TEST_SLOW=1 runs it "
+                           "(log of the last run: profiles/r2_cfg4_R10.txt)")
+def test_config4_full_size_at_the_configs_ten_images(fe):
+    """Config 4 with the config's own image count R = 10 (the quick test above cuts the sum at R = 2)."""
+    w = fi.config4(pbc_images=10)
+    o = orc.Oracle(oracle_problem(w), elec="fft")
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    for terms in (fi.TERM_ELEC, fi.TERM_ALL):
+        assert rel_l2(g.rhs(P, terms).cpu().numpy()[0], o.rhs(w.P0[0], terms)) < 1e-10, terms
     g.close()

@@ -140,3 +140,27 @@ def test_time_dependent_field_all_integrators(fe):
     assert np.allclose(e[:5], o1.energy(want)[:5], rtol=1e-9, atol=1e-11)
     g.close()
     g1.close()
+
+
+@pytest.mark.parametrize("bad", [float("nan"), float("inf")])
+def test_rk45_nonfinite_state_is_refused_not_accepted(fe, bad):
+    """A NaN / Inf cell makes the embedded error estimate non-finite.  fmax-style reductions drop NaN and would accept
+    the step with err = 0; the library must reject every attempt and return FE_ENONFINITE, leaving P as it was."""
+    w = workload_from_random(85, (8, 8, 4), (0, 0, 0), (0, 0, 0), batch=2)
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P0 = w.P0.copy()
+    act = np.argwhere(oracle_problem(w, 1).active)[3]
+    P0[1, 2, act[0], act[1], act[2]] = bad
+    P = g.state(P0)
+    with pytest.raises(fe.FeError) as ei:
+        g.step_rk45(P, 0.4, 0.05, 1e-6, 1000, fi.TERM_ALL)
+    assert ei.value.status == fe.FE_ENONFINITE
+    got = P.cpu().numpy()
+    assert np.array_equal(got[0], P0[0]) and np.array_equal(np.isnan(got[1]), np.isnan(P0[1]))
+    # every cell NaN: the maximum over the finite cells would be 0
+    P = g.state(np.full_like(w.P0, np.nan))
+    with pytest.raises(fe.FeError) as ei:
+        g.step_rk45(P, 0.4, 0.05, 1e-6, 1000, fi.TERM_ALL)
+    assert ei.value.status == fe.FE_ENONFINITE
+    g.close()
