@@ -146,6 +146,9 @@ def moved_bytes(w: fi.Workload, rsz: int):
         "yinv": B * 3 * (nz * ny * Lx * c + nz * m[1] * Lx * c),
         "xinv": B * 3 * (N * rsz + nz * ny * Lx * c),
         "local": B * 3 * N * rsz * 3,          # read P, read E_elec, write P_new
+        # fused x + y passes: the half spectrum S1 stays in L2 (ring of planes), only P in and S2 out touch HBM
+        "xyfwd": B * 3 * (N * rsz + nz * m[1] * Lx * c),
+        "xyinv": B * 3 * (N * rsz + nz * m[1] * Lx * c),
     }
 
 
@@ -228,6 +231,9 @@ def run_cuda(args):
     w = make_workload(args.workload, args.dtype)
     rsz = 8 if args.dtype == "f64" else 4
     g = fe.Grid.from_workload(w, device=dev, dtype=args.dtype)
+    g.set_option(fe.FE_OPT_FUSE_XY, args.fuse_xy)
+    if args.xy_ring:
+        g.set_option(fe.FE_OPT_XY_RING, args.xy_ring)
     t0 = time.time()
     g.precompute_tensor()
     t_pre = time.time() - t0
@@ -272,6 +278,7 @@ def run_cuda(args):
     prof = g.profile_read()
     g.profile(False)
     alg = moved_bytes(w, rsz)
+    alg = {k: v for k, v in alg.items() if prof.get(k, (0, 0))[1]}          # the kernels that actually ran
     pk, pk_kind = peaks()
     hbm = pk["hbm_gbs"]
     unit = measure_unit_peaks(torch, dev) if rank == 0 else {}
@@ -294,7 +301,7 @@ def run_cuda(args):
     traffic = cdom.get("dram_bytes") if cdom else (ctr.get(dom) if not isinstance(ctr.get(dom), dict) else None)
     # kernel that serves the profile slot on the size-specialised path (every bench workload but cfg1 takes it)
     fast_names = {"xfwd": "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>", "xinv": "k2_xinv",
-                  "local": "k_local2"}
+                  "local": "k_local2", "xyfwd": "k_xyfwd", "xyinv": "k_xyinv"}
     generic = args.workload == "cfg1"
     # which roofline binds the dominant kernel: the largest of its fractions of the three measured unit peaks
     fr = {"hbm": kern[dom]["frac_hbm"], "alu": kern[dom].get("frac_fp64", 0.0), "lds": kern[dom].get("frac_lds", 0.0)}
@@ -376,7 +383,7 @@ def run_cuda(args):
     if rank == 0 and not args.no_cufft:
         try:
             cufft = cufft_pipeline_ms(torch, w, args.dtype, dev)
-            ours = sum(kern[k]["ms"] for k in ("xfwd", "yfwd", "zmul", "yinv", "xinv") if k in kern)
+            ours = sum(kern[k]["ms"] for k in ("xfwd", "yfwd", "xyfwd", "zmul", "yinv", "xinv", "xyinv") if k in kern)
             cufft["ours_ms"] = ours
             cufft["speedup"] = cufft["ms_tight"] / ours
             cufft["speedup_vs_eager"] = cufft["ms_eager"] / ours
@@ -396,7 +403,7 @@ def run_cuda(args):
                 "config": {"workload": w.name, "grid": list(w.n), "batch": w.batch, "integrator": "euler",
                            "terms": "landau+gradient+elec+ext", "padded_fft": padded_dims(w),
                            "l2": "state and spectra exceed L2 (P 3N reals, spectra >= 4x that)",
-                           "parallelism": "replicas x%d" % world},
+                           "parallelism": "replicas x%d" % world, "fuse_xy": args.fuse_xy},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                 "clocks": cs.summary(), "cufft_baseline": cufft, "precompute_s": t_pre,
                 "energy_after": {"F_tot": float(en[4]), "finite": bool(np.isfinite(en).all())}}
@@ -552,6 +559,9 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison leg")
+    ap.add_argument("--fuse-xy", type=int, default=1, choices=[0, 1],
+                    help="FE_OPT_FUSE_XY: 1 = x and y passes fused through the L2 ring (default), 0 = separate kernels")
+    ap.add_argument("--xy-ring", type=int, default=0, help="FE_OPT_XY_RING (0 = automatic)")
     args = ap.parse_args()
     args.warmup_requested = args.warmup
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup

@@ -104,6 +104,21 @@ fe_status fe_get_time(const fe_grid* g, double* t);
  * NULL = all cells material 0.  Borrowed (not copied) until the next call or fe_destroy_grid.  PAPER.md:117. */
 fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map);
 
+/* Execution options (none changes what is computed; every value of every option is covered by the parity tests).
+ *   FE_OPT_FUSE_XY     1: the forward x and y transforms run in ONE cooperative kernel that hands the half spectra over
+ *                      through a ring of planes resident in L2 whenever the geometry allows it
+ *                      (open x and y, 2 ny = padded y length 256 or 512, padded x length 256 or 512);
+ *                      0 (default): the separate x and y kernels with the half spectrum in HBM between them.  Measured
+ *                      on B200: the fused kernel moves 1.2 GB instead of 1.8 GB of DRAM traffic at config 5a but is
+ *                      slower (both passes are bound by shared-memory throughput on the SM).
+ *   FE_OPT_XY_TIMEOUTS read-only (fe_get_option synchronises the device): 1 if a wait inside the fused kernel ever
+ *                      timed out (it cannot unless the device is shared with a kernel that never yields).
+ *   FE_OPT_XY_RING     planes in the L2 ring of the fused pass; 0 (default) sizes it from the geometry (>= 24 planes,
+ *                      <= 32 MB), 2..4096 fixes it (clamped to the number of planes). */
+enum { FE_OPT_FUSE_XY = 0, FE_OPT_XY_TIMEOUTS = 1, FE_OPT_XY_RING = 2 };
+fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value);
+fe_status fe_get_option(fe_grid* g, int32_t option, int32_t* value);
+
 /* a0: cell-averaged dipolar tensor K_ij(d) on the padded box and its real spectrum (once per
  * geometry).  PAPER.md:76,115; readings A3, A4. */
 fe_status fe_precompute_tensor(fe_grid* g, void* cuda_stream);
@@ -151,8 +166,8 @@ uint64_t  fe_launch_count(const fe_grid* g);
 /* Per-kernel timing for the roofline report: while enabled, fe_rhs/fe_step record a CUDA event on the
  * stream before every kernel launch.  fe_profile_read synchronises the stream and returns, per kernel
  * kind {0 x-forward, 1 y-forward, 2 fused z + tensor multiply, 3 y-inverse, 4 x-inverse, 5 local step,
- * 6 other}, the summed device time in ms (host_ms[7]) and the launch count (host_counts[7]) since the last
- * read, then clears the record. */
+ * 6 other, 7 fused x+y forward, 8 fused y+x inverse}, the summed device time in ms (host_ms[9]) and the launch
+ * count (host_counts[9]) since the last read, then clears the record. */
 fe_status fe_profile(fe_grid* g, int32_t enable);
 fe_status fe_profile_read(fe_grid* g, double* host_ms, uint64_t* host_counts, void* cuda_stream);
 

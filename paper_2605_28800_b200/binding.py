@@ -24,8 +24,9 @@ SYMBOLS = ["fe_create_grid", "fe_destroy_grid", "fe_workspace_bytes", "fe_bind_w
            "fe_set_global", "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs",
            "fe_step", "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_launch_count", "fe_last_error",
            "fe_version", "fe_profile", "fe_profile_read", "fe_step_rk45", "fe_set_external_wave", "fe_set_time",
-           "fe_get_time"]
-KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other"]
+           "fe_get_time", "fe_set_option", "fe_get_option"]
+KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other", "xyfwd", "xyinv"]
+FE_OPT_FUSE_XY, FE_OPT_XY_TIMEOUTS, FE_OPT_XY_RING = 0, 1, 2
 
 
 class fe_rk45_stats(ctypes.Structure):
@@ -96,12 +97,15 @@ def load():
         L.fe_set_time.argtypes = [vp, dbl]
         L.fe_get_time.argtypes = [vp, ctypes.POINTER(dbl)]
         L.fe_step_rk45.argtypes = [vp, vp, dbl, dbl, dbl, i32, u32, ctypes.POINTER(fe_rk45_stats), vp]
+        L.fe_set_option.argtypes = [vp, i32, i32]
+        L.fe_get_option.argtypes = [vp, i32, ctypes.POINTER(i32)]
         L.fe_launch_count.restype = ctypes.c_uint64
         L.fe_last_error.restype = ctypes.c_char_p
         L.fe_version.restype = ctypes.c_char_p
         for name in ("fe_create_grid", "fe_destroy_grid", "fe_bind_workspace", "fe_set_material", "fe_set_global",
                      "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs", "fe_step",
-                     "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_profile", "fe_profile_read"):
+                     "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_profile", "fe_profile_read", "fe_set_option",
+                     "fe_get_option"):
             getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -234,10 +238,20 @@ def fe_profile(h, enable: bool):
 
 def fe_profile_read(h):
     """{kind: (total ms, launches)} since the last read."""
-    ms = (ctypes.c_double * 7)()
-    cnt = (ctypes.c_uint64 * 7)()
+    ms = (ctypes.c_double * len(KERNEL_KINDS))()
+    cnt = (ctypes.c_uint64 * len(KERNEL_KINDS))()
     _check(load().fe_profile_read(h, ms, cnt, _stream()))
     return {k: (ms[i], int(cnt[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
+def fe_set_option(h, option: int, value: int):
+    _check(load().fe_set_option(h, int(option), int(value)))
+
+
+def fe_get_option(h, option: int) -> int:
+    v = ctypes.c_int32(0)
+    _check(load().fe_get_option(h, int(option), ctypes.byref(v)))
+    return int(v.value)
 
 
 def fe_launch_count(h) -> int:
@@ -330,6 +344,8 @@ class Grid:
 
     def get_tensor(self) -> np.ndarray: return fe_get_tensor(self.h)
     def launch_count(self) -> int: return fe_launch_count(self.h)
+    def set_option(self, option: int, value: int): fe_set_option(self.h, option, value)
+    def get_option(self, option: int) -> int: return fe_get_option(self.h, option)
     def profile(self, enable: bool): fe_profile(self.h, enable)
     def profile_read(self): return fe_profile_read(self.h)
 

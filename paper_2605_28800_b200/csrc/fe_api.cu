@@ -58,7 +58,9 @@ struct fe_grid {
     // workspace (borrowed)
     unsigned char* ws;
     size_t ws_bytes;
-    size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_K[6], o_part, o_box, o_Sbox, total_bytes;
+    size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_K[6], o_part, o_cnt, o_box, o_Sbox, total_bytes;
+    int opt_fuse_xy;                 // FE_OPT_FUSE_XY
+    int opt_xy_ring;                 // FE_OPT_XY_RING (0: automatic)
     int nblk;
     bool tensor_ready;
     bool fast[3];                    // size-specialised register FFT kernels available for the x / y / z pass
@@ -80,7 +82,7 @@ struct fe_grid {
     size_t prof_used;
 };
 
-enum { K_XFWD = 0, K_YFWD, K_ZMUL, K_YINV, K_XINV, K_LOCAL, K_OTHER, K_NKINDS };
+enum { K_XFWD = 0, K_YFWD, K_ZMUL, K_YINV, K_XINV, K_LOCAL, K_OTHER, K_XYFWD, K_XYINV, K_NKINDS };
 
 // record an event on the stream before a launch of `kind` (kind < 0: closes the previous interval)
 static void mark(fe_grid* g, int kind, cudaStream_t st)
@@ -168,6 +170,7 @@ static void layout_workspace(fe_grid* g)
     off = hot1 > s ? hot1 : s;
     g->nblk = 296;
     g->o_part = off; off += align_up((size_t)B * g->nblk * 8 * sizeof(double));
+    g->o_cnt = off;  off += align_up(((size_t)2 * B * 3 * q.n[2] + 1) * sizeof(int));     // plane counters of the fused x+y pass
     g->total_bytes = off;
 }
 
@@ -240,6 +243,8 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     }
     g->dirty = true;
     g->mixed = 0;
+    g->opt_fuse_xy = 0;
+    g->opt_xy_ring = 0;
     g->map = nullptr;
     g->ws = nullptr;
     g->ws_bytes = 0;
@@ -450,6 +455,40 @@ extern "C" fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map)
     return FE_OK;
 }
 
+extern "C" fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value)
+{
+    if (!g) return fail(FE_EINVAL, "null argument");
+    if (option == FE_OPT_FUSE_XY && (value == 0 || value == 1)) {
+        g->opt_fuse_xy = value;
+        g->gvalid = false;               // a captured graph holds the other kernels
+        return FE_OK;
+    }
+    if (option == FE_OPT_XY_RING && value >= 0 && value <= 4096) {
+        g->opt_xy_ring = value;
+        g->gvalid = false;
+        return FE_OK;
+    }
+    return fail(FE_EINVAL, "unknown option %d or bad value %d", option, value);
+}
+
+extern "C" fe_status fe_get_option(fe_grid* g, int32_t option, int32_t* value)
+{
+    if (!g || !value) return fail(FE_EINVAL, "null argument");
+    if (option == FE_OPT_FUSE_XY) { *value = g->opt_fuse_xy; return FE_OK; }
+    if (option == FE_OPT_XY_RING) { *value = g->opt_xy_ring; return FE_OK; }
+    if (option == FE_OPT_XY_TIMEOUTS) {
+        *value = 0;
+        if (!g->ws) return FE_OK;
+        int flag = 0;
+        FE_CUDA(cudaDeviceSynchronize());
+        const int nplanes = g->desc.batch * 3 * g->geo.n[2];
+        FE_CUDA(cudaMemcpy(&flag, g->ws + g->o_cnt + (size_t)2 * nplanes * sizeof(int), sizeof(int), cudaMemcpyDeviceToHost));
+        *value = flag != 0;
+        return FE_OK;
+    }
+    return fail(FE_EINVAL, "unknown option %d", option);
+}
+
 static fe_status sync_params(fe_grid* g, cudaStream_t st)
 {
     const int B = g->desc.batch, M = g->desc.n_materials;
@@ -566,6 +605,26 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     if (use4) axis4_radices(My, perm);
     const int64_t ks[4] = {(int64_t)Hz * Hy * p, tl ? L : (int64_t)Hy * p, tl ? (int64_t)Hz * L : p,
                            tl ? (int64_t)Hy * Hz * L : L};
+    // x + y passes in one cooperative kernel, S1 planes handed over through a ring that stays in L2 (NEXT-2)
+    const bool fuse = use4 && g->opt_fuse_xy && xy_supported(q.m[0] / 2, My, nx, ny);
+    // ring: deep enough for every block's X group to run one task ahead of the plane being read (148 blocks / row
+    // groups per plane), at least 24 planes, at most 32 MB (it must stay in L2) -- or the caller's FE_OPT_XY_RING
+    int ring_slots = g->opt_xy_ring;
+    if (ring_slots <= 0) {
+        const int rows_task = q.m[0] / 2 >= 256 ? 16 : 32;
+        const int64_t plane_bytes = (int64_t)G * ny * 128;
+        ring_slots = 3 * (148 * rows_task / ny + 1);
+        if (ring_slots < 24) ring_slots = 24;
+        while (ring_slots > 8 && ring_slots * plane_bytes > (32ll << 20)) ring_slots /= 2;
+    }
+    if (ring_slots > slabs) ring_slots = slabs;
+    if (ring_slots < 2) ring_slots = 2;
+    if (fuse) {
+        mark(g, K_XYFWD, st);
+        FE_CUDA(launch_xyfwd<T>(g->ctx, Y, S1, S2, nx, ny, nz, slabs, G, ring_slots, y2_sz, y2_sg, y2_sb,
+                                reinterpret_cast<int*>(g->ws + g->o_cnt), st));
+        g->launches += 2;            // counter reset + kernel
+    } else {
     mark(g, K_XFWD, st);
     if (g->fast[0]) FE_CUDA(launch_xfwd2<T>(g->ctx, Y, S1, nx, rows, nx, xspec, L, st));
     else FE_CUDA(launch_xfwd<T>(g->ctx, Y, S1, q.n[0], q.n[1], slabs, q.n[0], (int64_t)q.n[0] * q.n[1], p, p * q.n[1], st));
@@ -580,6 +639,8 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     } else {
         FE_CUDA(launch_axis<T>(g->ctx, 1, -1, S1, S2, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.n[1],
                                p * q.n[1] * q.n[2], p, p * q.m[1], p * q.m[1] * q.n[2], st));
+    }
+    g->launches += 2;
     }
     mark(g, K_ZMUL, st);
     if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, st));
@@ -598,7 +659,7 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     mark(g, K_XINV, st);
     if (g->fast[0]) FE_CUDA(launch_xinv2<T>(g->ctx, S1, E, nx, rows, nx, xspec, L, st));
     else FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
-    g->launches += 5;
+    g->launches += 3;
     return FE_OK;
 }
 

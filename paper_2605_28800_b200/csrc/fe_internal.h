@@ -133,6 +133,11 @@ cudaError_t launch_zmul2(const FftCtx& c, void* S, const T* Kt, const DevMember*
                          int batch, const int64_t sstr[4] /* cs, s_z, s_ky, s_g */,
                          const int64_t kstr[4] /* kcs, k_skz, k_sky, k_sg */,
                          const int perm[3] /* slot-order radices of ky, {0,0,0}: natural */, cudaStream_t st);
+// x and y passes fused through an L2-resident ring of S1 planes (fe_fft2_xy.cu).  counters: 2 * nplanes + 1 ints.
+bool xy_supported(int Mx, int My, int nx, int ny);
+template <typename T>
+cudaError_t launch_xyfwd(const FftCtx& c, const T* P, void* ring, void* S2, int nx, int ny, int nz, int nplanes, int G,
+                         int ring_slots, int64_t s2_sz, int64_t s2_sg, int64_t s2_sb, int* counters, cudaStream_t st);
 cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
 
 // ---- tensor (fe_tensor.cu) --------------------------------------------------------------------

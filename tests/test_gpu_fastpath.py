@@ -255,3 +255,45 @@ def test_odd_open_x_axis_is_refused(fe):
     assert ei.value.status == fe.FE_EINVAL
     with pytest.raises(fe.FeError):
         fe.Grid((12, 8, 8), (1.0, 1.0, 1.0), periodic=(1, 0, 0))      # periodic axes stay powers of two
+
+
+@pytest.mark.parametrize("n,batch,dtype", [
+    ((128, 128, 32), 2, "f64"),        # x 128p, y 256p: ROWS = 32 per X task, 192 planes through a ring of 24
+    ((256, 256, 32), 1, "f64"),        # x 256p, y 512p: the kernels of config 5a
+    ((200, 128, 32), 1, "f64"),        # partial pruning on x (200 of 256 reals)
+    ((256, 256, 32), 1, "f32"),
+])
+def test_fused_xy_pass_through_the_l2_ring(fe, n, batch, dtype):
+    """FE_OPT_FUSE_XY: x and y passes in one cooperative kernel, half spectra handed over through a
+    ring of planes.  Both settings of the option against oracle-FFT, against each other, over many steps (the ring and its
+    counters are reused by every launch) and under CUDA-graph replay; no wait may ever time out."""
+    w = _workload(n, batch=batch)
+    tol = TOL_RHS64 if dtype == "f64" else TOL32
+    P0 = w.P0 if dtype == "f64" else w.P0.astype(np.float32).astype(np.float64)
+    o = orc.Oracle(oracle_problem(w, batch - 1), elec="fft")
+    want = o.rhs(P0[batch - 1], fi.TERM_ELEC)
+    g = fe.Grid.from_workload(w, dtype=dtype)
+    g.precompute_tensor()
+    P = g.state(P0)
+    res = {}
+    for fuse in (1, 0):
+        g.set_option(fe.FE_OPT_FUSE_XY, fuse)
+        assert g.get_option(fe.FE_OPT_FUSE_XY) == fuse
+        g.profile(True)
+        res[fuse] = g.rhs(P, fi.TERM_ELEC).cpu().numpy().astype(np.float64)
+        kinds = {k for k, (ms, cnt) in g.profile_read().items() if cnt}
+        g.profile(False)
+        assert ("xyfwd" in kinds) == bool(fuse) and ("xfwd" in kinds) == (not fuse)
+        assert rel_l2(res[fuse][batch - 1], want) < tol
+    assert rel_l2(res[1], res[0]) < (1e-13 if dtype == "f64" else 1e-5)
+    # 40 Euler steps in one call (graph replay) with the fused pass against 40 single steps without it
+    g.set_option(fe.FE_OPT_FUSE_XY, 1)
+    Pa = g.state(P0)
+    g.step(Pa, w.dt, 40, fi.EULER, fi.TERM_ALL)
+    g.set_option(fe.FE_OPT_FUSE_XY, 0)
+    Pb = g.state(P0)
+    for _ in range(40):
+        g.step(Pb, w.dt, 1, fi.EULER, fi.TERM_ALL)
+    assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < (1e-12 if dtype == "f64" else 1e-4)
+    assert g.get_option(fe.FE_OPT_XY_TIMEOUTS) == 0
+    g.close()
