@@ -562,7 +562,7 @@ def main():
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison leg")
     ap.add_argument("--fuse-xy", type=int, default=0, choices=[0, 1],
                     help="FE_OPT_FUSE_XY: 1 = x and y passes fused through the L2 ring, 0 = separate kernels (default)")
-    ap.add_argument("--z-pairs", type=int, default=0, choices=[0, 1], help="FE_OPT_Z_PAIRS")
+    ap.add_argument("--z-pairs", type=int, default=0, choices=[0, 1, 2], help="FE_OPT_Z_PAIRS")
     ap.add_argument("--xy-ring", type=int, default=0, help="FE_OPT_XY_RING (0 = automatic)")
     args = ap.parse_args()
     args.warmup_requested = args.warmup

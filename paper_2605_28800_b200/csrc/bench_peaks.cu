@@ -86,6 +86,47 @@ __global__ void __launch_bounds__(256) k_kmul(const T* __restrict__ P, const T* 
     }
 }
 
+// warps 0-3 of a block run the DFMA chains, warps 4-7 the shared-memory loads: mode 1 = fp64 only, 2 = loads only,
+// 3 = both at once.  If the two units are independent, mode 3 takes max(mode 1, mode 2); if they share a resource, the sum.
+__global__ void __launch_bounds__(256) k_mix(double* out, int iters, double a, double b, int mode)
+{
+    __shared__ double2 buf[2048];
+    for (int i = threadIdx.x; i < 2048; i += 256) buf[i] = make_double2((double)i, 1.0);
+    __syncthreads();
+    const int warp = threadIdx.x >> 5;
+    double s = 0.0;
+    if (warp < 4) {
+        if (mode & 1) {
+            double v[kChains];
+#pragma unroll
+            for (int c = 0; c < kChains; ++c) v[c] = (double)(threadIdx.x + c) * 1e-3;
+            for (int i = 0; i < iters; ++i) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+#pragma unroll
+                    for (int c = 0; c < kChains; ++c) v[c] = fma(v[c], a, b);
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < kChains; ++c) s += v[c];
+        }
+    } else if (mode & 2) {
+        double2 acc = make_double2(0.0, 0.0);
+        int idx = threadIdx.x;
+        for (int i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const double2 v = buf[(idx + u * 256) & 2047];
+                acc.x += v.x;      // two DADD per load: small against the 4 wavefronts of the load
+                acc.y += v.y;
+            }
+            idx = (idx + 8) & 2047;
+        }
+        s = acc.x + acc.y;
+    }
+    if (s == 12345.678) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 struct Timer {
     cudaEvent_t e0, e1;
     Timer() { cudaEventCreate(&e0); cudaEventCreate(&e1); }
@@ -129,6 +170,26 @@ extern "C" int fe_peak_fp64(void* scratch, int blocks_per_sm, int iters, double*
         if (rep > 0 && r > best) best = r;
     }
     *out_inst_per_s = best;
+    return 0;
+}
+
+// out_ms[3]: time of k_mix in mode 1 (fp64 on half the warps), 2 (shared-memory loads on the other half), 3 (both)
+extern "C" int fe_peak_mix(void* scratch, int iters, double* out_ms, void* stream)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int grid = sm_count();
+    Timer t;
+    for (int mode = 1; mode <= 3; ++mode) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 3; ++rep) {
+            t.start(st);
+            k_mix<<<grid, 256, 0, st>>>(static_cast<double*>(scratch), iters, 0.999999, 1e-7, mode);
+            const float ms = t.stop(st);
+            if (cudaGetLastError() != cudaSuccess || ms <= 0.f) return 1;
+            if (rep > 0 && ms < best) best = ms;
+        }
+        out_ms[mode - 1] = best;
+    }
     return 0;
 }
 

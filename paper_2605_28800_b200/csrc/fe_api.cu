@@ -465,7 +465,7 @@ extern "C" fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value)
         g->gvalid = false;               // a captured graph holds the other kernels
         return FE_OK;
     }
-    if (option == FE_OPT_Z_PAIRS && (value == 0 || value == 1)) {
+    if (option == FE_OPT_Z_PAIRS && value >= 0 && value <= 2) {
         g->opt_z_pairs = value;
         g->gvalid = false;
         return FE_OK;
@@ -652,7 +652,7 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     }
     mark(g, K_ZMUL, st);
     if (g->fast[2] && g->opt_z_pairs && zmul3_supported(q.m[2], nz))
-        FE_CUDA(launch_zmul3<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, st));
+        FE_CUDA(launch_zmul3<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, g->opt_z_pairs, st));
     else if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, st));
     else FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
     mark(g, K_YINV, st);

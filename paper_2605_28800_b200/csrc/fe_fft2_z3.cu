@@ -253,6 +253,243 @@ __global__ void __launch_bounds__(Z3Cfg<T>::THREADS, 1) k3_zmul(cx<T>* S, const 
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------------------------
+// k5_zmul: ONE tile at a time with the in-place column layout above, cp.async staging of the next tile's rows and the
+// K~ tile of the item in shared memory (as k2_zmul).  Per tile two phases and two block barriers:
+//   M phase  8-point step + multiply + inverse 8-point step of the current tile, every thread its k1, in place;
+//   E phase  inverse 32-point step of the current tile (column -> global rows) and forward 32-point step of the NEXT
+//            tile (staged rows -> the same column): 2 CQT warp tasks on NW warps.  Warp w < NW/2 does both steps of
+//            column group w; the remaining NW/4 groups have their inverse step done by warps NW/2 .. and their forward
+//            step by the last NW/4 warps (ordered by a two-warp barrier): every scheduler gets three 32-point tasks,
+//            where the three-phase kernel gives two of the four schedulers four.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename T> struct Z5Cfg {
+    static constexpr int M = 256, R1 = 32, R2 = 8, HZ = M / 2 + 1, NIN = M / 2;
+    static constexpr int LANES = 128 / (int)sizeof(cx<T>);
+    static constexpr int THREADS = LANES * R1;
+    static constexpr int NW = THREADS / 32, HALF = NW / 2, Q = NW / 4;
+    static constexpr int TPW = 32 / LANES;
+    static constexpr int CQT = 3 * R2 / TPW;
+    static constexpr int TILE = 3 * M * LANES;
+    static constexpr size_t ex_bytes = (size_t)TILE * sizeof(cx<T>);
+    static constexpr size_t st_bytes = (size_t)3 * NIN * LANES * sizeof(cx<T>);
+    static constexpr size_t k_bytes = ((size_t)6 * HZ * LANES * sizeof(T) + 15) / 16 * 16;
+    static constexpr size_t tw_bytes = (size_t)(R2 - 1) * R1 * sizeof(cx<T>);       // w_M^(n2 k1) at [n2 - 1][k1]
+    static constexpr size_t smem = ex_bytes + st_bytes + k_bytes + tw_bytes;
+    static_assert(CQT == HALF + Q, "24 columns x LANES = HALF + Q column groups");
+};
+
+__device__ __forceinline__ void z5_cp16(void* smem, const void* gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void z5_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+__device__ __forceinline__ void z5_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+
+struct Z5It {
+    int item, b, m;
+};
+
+template <typename T, bool FULLZ>
+__global__ void __launch_bounds__(Z5Cfg<T>::THREADS, 1) k5_zmul(cx<T>* S, const T* __restrict__ Kt, Z3Args a)
+{
+    using C = Z5Cfg<T>;
+    constexpr int M = C::M, R1 = C::R1, R2 = C::R2, LANES = C::LANES, NW = C::NW, HALF = C::HALF, Q = C::Q, TPW = C::TPW;
+    constexpr int HZ = C::HZ, NIN = C::NIN;
+    cx<T>* buf = reinterpret_cast<cx<T>*>(fe2_smem);                       // exchange [3][k1 * 8 + n2][LANES]
+    cx<T>* stage = buf + C::TILE;                                          // staged rows [3][NIN][LANES]
+    T* kbuf = reinterpret_cast<T*>(stage + 3 * NIN * LANES);               // K~ tile [6][HZ][LANES]
+    cx<T>* twk = reinterpret_cast<cx<T>*>(reinterpret_cast<unsigned char*>(kbuf) + C::k_bytes);   // [R2 - 1][R1]
+    const int lane = threadIdx.x % LANES, tp = threadIdx.x / LANES, warp = threadIdx.x / 32, sub = tp % TPW;
+    const int64_t cs = a.cs, sz = a.s_z;
+    const int nitems = a.ngroups * (a.My / 2 + 1);
+
+    auto valid = [&](const Z5It& it) { return it.item < nitems; };
+    auto mirrors = [&](int item) {
+        const int kyh = item / a.ngroups;
+        return (kyh == 0 || 2 * kyh == a.My) ? 1 : 2;
+    };
+    auto advance = [&](Z5It it) {
+        if (++it.m < mirrors(it.item)) return it;
+        it.m = 0;
+        if (++it.b < a.batch) return it;
+        it.b = 0;
+        it.item += gridDim.x;
+        return it;
+    };
+    auto tile_base = [&](const Z5It& it) -> cx<T>* {
+        const int kyh = it.item / a.ngroups, kxg = it.item - kyh * a.ngroups;
+        const int ky = it.m ? a.My - kyh : kyh;
+        int slot = ky;
+        if (a.la >= 0)
+            slot = ((ky & ((1 << a.la) - 1)) << (a.lb + a.lc)) | (((ky >> a.la) & ((1 << a.lb) - 1)) << a.lc) |
+                   (ky >> (a.la + a.lb));
+        return S + (int64_t)it.b * 3 * cs + (int64_t)slot * a.s_ky + (int64_t)kxg * a.s_g;
+    };
+    // asynchronous copies: data rows of a tile -> stage, K~ tile of an item -> kbuf (16 bytes per copy)
+    auto prefetch_tile = [&](const cx<T>* tb) {
+        constexpr int PER = 16 / (int)sizeof(cx<T>), OPS_ROW = LANES / PER, RSTEP = C::THREADS / OPS_ROW;
+        static_assert(NIN % RSTEP == 0, "tile copy must be regular");
+        const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
+        const cx<T>* g = tb + (int64_t)row0 * sz + q * PER;
+        cx<T>* s = stage + row0 * LANES + q * PER;
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int j = 0; j < NIN / RSTEP; ++j)
+                if (FULLZ || row0 + j * RSTEP < a.nz)
+                    z5_cp16(s + (c * NIN + j * RSTEP) * LANES, g + c * cs + (int64_t)(j * RSTEP) * sz);
+    };
+    auto prefetch_k = [&](int item) {
+        constexpr int PER = 16 / (int)sizeof(T), OPS_ROW = LANES / PER, RSTEP = C::THREADS / OPS_ROW;
+        const int kyh = item / a.ngroups, kxg = item - kyh * a.ngroups;
+        const int q = threadIdx.x % OPS_ROW, row0 = threadIdx.x / OPS_ROW;
+        const T* g = Kt + (int64_t)kyh * a.k_sky + (int64_t)kxg * a.k_sg + (int64_t)row0 * a.k_skz + q * PER;
+        T* s = kbuf + row0 * LANES + q * PER;
+#pragma unroll
+        for (int c6 = 0; c6 < 6; ++c6)
+#pragma unroll
+            for (int j = 0; j < (HZ + RSTEP - 1) / RSTEP; ++j)
+                if (row0 + j * RSTEP < HZ)
+                    z5_cp16(s + (c6 * HZ + j * RSTEP) * LANES, g + c6 * a.kcs + (int64_t)(j * RSTEP) * a.k_skz);
+    };
+    // inverse 32-point step of column group q of the current tile: exchange column -> rows of the tile in memory
+    auto taskU = [&](cx<T>* tb, int q) {
+        const int col = q * TPW + sub, c = col >> 3, n2 = col & 7;
+        const cx<T>* src = buf + (c * M + n2) * LANES + lane;
+        cx<T> w[R1];
+        static_for<R1>([&](auto pc) { w[decltype(pc)::value] = src[brev<R1>(decltype(pc)::value) * R2 * LANES]; });
+        DitF<T, +1, R1, 0, false, true>::run(w);
+        cx<T>* out = tb + lane + c * cs + (int64_t)n2 * sz;
+        static_for<R1 / 2>([&](auto nc) {
+            constexpr int n1 = decltype(nc)::value;
+            if (FULLZ || R2 * n1 + n2 < a.nz) out[(int64_t)(R2 * n1) * sz] = w[n1];
+        });
+    };
+    // forward 32-point step of column group q of the next tile: staged rows -> exchange column
+    auto taskT = [&](int q) {
+        const int col = q * TPW + sub, c = col >> 3, n2 = col & 7;
+        const cx<T>* src = stage + (c * NIN + n2) * LANES + lane;
+        cx<T> w[R1];
+        static_for<R1>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int n1 = brev<R1>(p);
+            if constexpr (n1 < R1 / 2) w[p] = src[n1 * R2 * LANES];
+        });
+        DitF<T, -1, R1, 0, true, false>::run(w);
+        cx<T>* dst = buf + (c * M + n2) * LANES + lane;
+        static_for<R1>([&](auto kc) { dst[decltype(kc)::value * R2 * LANES] = w[decltype(kc)::value]; });
+    };
+    const int k1 = tp;
+    auto phaseM = [&](const Z5It& it, const T esc) {
+        cx<T> wk[R2];
+        static_for<R2 - 1>([&](auto nc) { wk[decltype(nc)::value + 1] = twk[decltype(nc)::value * R1 + k1]; });
+        const unsigned sy = it.m ? 0x80000000u : 0u;          // mirror tile: ky > My / 2, xy and yz change sign
+        cx<T>* row = buf + (k1 * R2) * LANES + lane;
+        cx<T> u[3][R2];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            static_for<R2>([&](auto nc) { u[c][decltype(nc)::value] = row[(c * M + decltype(nc)::value) * LANES]; });
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            static_for<R2 - 1>([&](auto nc) {
+                constexpr int n2 = decltype(nc)::value + 1;
+                u[c][n2] = cmul(u[c][n2], wk[n2]);
+            });
+            Dif<T, -1, R2>::run(u[c]);
+        }
+        static_for<R2>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int k2 = brev<R2>(p);
+            const int kz = k1 + R1 * k2;
+            const int kzm = 2 * kz <= M ? kz : M - kz;
+            const unsigned sgn = 2 * kz > M ? 0x80000000u : 0u;
+            const T* kp = kbuf + kzm * LANES + lane;
+            const T Kxx = kp[0], Kyy = kp[HZ * LANES], Kzz = kp[2 * HZ * LANES];
+            const T Kxy = z3_xorsign(kp[3 * HZ * LANES], sy), Kxz = z3_xorsign(kp[4 * HZ * LANES], sgn);
+            const T Kyz = z3_xorsign(kp[5 * HZ * LANES], sy ^ sgn);
+            const cx<T> Px = u[0][p], Py = u[1][p], Pz = u[2][p];
+            u[0][p] = {Kxx * Px.x + Kxy * Py.x + Kxz * Pz.x, Kxx * Px.y + Kxy * Py.y + Kxz * Pz.y};
+            u[1][p] = {Kxy * Px.x + Kyy * Py.x + Kyz * Pz.x, Kxy * Px.y + Kyy * Py.y + Kyz * Pz.y};
+            u[2][p] = {Kxz * Px.x + Kyz * Py.x + Kzz * Pz.x, Kxz * Px.y + Kyz * Py.y + Kzz * Pz.y};
+        });
+        // -1/(eps0 epsB) of Eq. 6 rides on the inverse twiddles
+        static_for<R2 - 1>([&](auto nc) {
+            constexpr int n2 = decltype(nc)::value + 1;
+            wk[n2] = {esc * wk[n2].x, esc * wk[n2].y};
+        });
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            DitF<T, +1, R2>::run(u[c]);
+            static_for<R2>([&](auto nc) {
+                constexpr int n2 = decltype(nc)::value;
+                cx<T> val = u[c][n2];
+                if constexpr (n2 != 0) val = cmulc(val, wk[n2]);
+                else val = {esc * val.x, esc * val.y};
+                row[(c * M + n2) * LANES] = val;
+            });
+        }
+    };
+
+    Z5It cur{(int)blockIdx.x, 0, 0};
+    if (!valid(cur)) return;
+    if (!FULLZ) {                           // rows nz .. M/2 of the staged half: cleared once, never written again
+        for (int e = threadIdx.x; e < 3 * NIN * LANES; e += C::THREADS) stage[e] = cx<T>{0, 0};
+        __syncthreads();
+    }
+    for (int e = threadIdx.x; e < (R2 - 1) * R1; e += C::THREADS)
+        twk[e] = static_cast<const cx<T>*>(a.tw)[((e / R1 + 1) * (e % R1)) * (kTwiddleN / M)];
+    cx<T>* cur_base = tile_base(cur);
+    T esc_cur = (T)(-a.members[cur.b].escale), esc_nxt = esc_cur;
+    prefetch_tile(cur_base);
+    prefetch_k(cur.item);
+    z5_commit();
+    z5_wait_all();
+    __syncthreads();
+    // prologue E phase: forward step of the first tile only
+    if (warp < HALF) taskT(warp);
+    else if (warp >= HALF + Q) taskT(warp - Q);
+    Z5It nxt = advance(cur);
+    cx<T>* nxt_base = valid(nxt) ? tile_base(nxt) : cur_base;
+    if (valid(nxt)) esc_nxt = (T)(-a.members[nxt.b].escale);
+    __syncthreads();
+    if (valid(nxt)) prefetch_tile(nxt_base);
+    z5_commit();
+    while (true) {
+        phaseM(cur, esc_cur);
+        z5_wait_all();                      // rows of the next tile have landed ...
+        __syncthreads();                    // ... for every thread; exchange holds the inverse-ready tile; K~ tile free
+        const bool more = valid(nxt);
+        if (more && nxt.item != cur.item) prefetch_k(nxt.item);
+        z5_commit();
+        if (warp < HALF) {
+            taskU(cur_base, warp);
+            if (more) taskT(warp);
+        } else if (warp < HALF + Q) {
+            taskU(cur_base, warp);
+            z3_arrive(1 + warp - HALF);
+        } else {
+            z3_sync(1 + warp - HALF - Q);
+            if (more) taskT(warp - Q);
+        }
+        if (!more) break;
+        cur = nxt;
+        cur_base = nxt_base;
+        esc_cur = esc_nxt;
+        nxt = advance(cur);
+        if (valid(nxt)) {
+            nxt_base = tile_base(nxt);
+            esc_nxt = (T)(-a.members[nxt.b].escale);
+        }
+        z5_wait_all();                      // K~ of the tile about to be multiplied
+        __syncthreads();                    // exchange holds the forward-ready tile; staging buffer free
+        if (valid(nxt)) prefetch_tile(nxt_base);
+        z5_commit();
+    }
+}
+
 }  // namespace v2
 
 // paired fused z pass; same argument meaning as launch_zmul2 (fe_fft2_z.cu).  Only the zero-padded 256-point axis.
@@ -260,7 +497,8 @@ bool zmul3_supported(int M, int nz) { return M == 256 && 2 * nz <= M; }
 
 template <typename T>
 cudaError_t launch_zmul3(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
-                         int batch, const int64_t sstr[4], const int64_t kstr[4], const int perm[3], cudaStream_t st)
+                         int batch, const int64_t sstr[4], const int64_t kstr[4], const int perm[3], int variant,
+                         cudaStream_t st)
 {
     using C = v2::Z3Cfg<T>;
     if (!zmul3_supported(c.plan[2].M, nz)) return cudaErrorInvalidValue;
@@ -288,14 +526,31 @@ cudaError_t launch_zmul3(const FftCtx& c, void* S, const T* Kt, const DevMember*
     v2::Z3Args a{c.tw, members, My, batch, nz, ngroups, nunits, sstr[0], sstr[1], sstr[2], sstr[3],
                  kstr[0], kstr[1], kstr[2], kstr[3], lg[0], lg[1], lg[2]};
     const int grid = nunits < nblocks ? nunits : nblocks;
+    if (variant == 2) {
+        using C5 = v2::Z5Cfg<T>;
+        static PerDevice<int> cache5;
+        int& conf = cache5.here();
+        if (!conf) {
+            cudaError_t e = cudaFuncSetAttribute(v2::k5_zmul<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C5::smem);
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(v2::k5_zmul<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C5::smem);
+            if (e != cudaSuccess) return e;
+            conf = 1;
+        }
+        const int nitems = ngroups * (My / 2 + 1);
+        const int grid5 = nitems < nblocks ? nitems : nblocks;
+        if (2 * nz == C5::M) v2::k5_zmul<T, true><<<grid5, C5::THREADS, C5::smem, st>>>(static_cast<v2::cx<T>*>(S), Kt, a);
+        else v2::k5_zmul<T, false><<<grid5, C5::THREADS, C5::smem, st>>>(static_cast<v2::cx<T>*>(S), Kt, a);
+        return cudaGetLastError();
+    }
     if (2 * nz == C::M) v2::k3_zmul<T, true><<<grid, C::THREADS, C::smem, st>>>(static_cast<v2::cx<T>*>(S), Kt, a);
     else v2::k3_zmul<T, false><<<grid, C::THREADS, C::smem, st>>>(static_cast<v2::cx<T>*>(S), Kt, a);
     return cudaGetLastError();
 }
 
 template cudaError_t launch_zmul3<double>(const FftCtx&, void*, const double*, const DevMember*, int, int, int, int,
-                                          const int64_t*, const int64_t*, const int*, cudaStream_t);
+                                          const int64_t*, const int64_t*, const int*, int, cudaStream_t);
 template cudaError_t launch_zmul3<float>(const FftCtx&, void*, const float*, const DevMember*, int, int, int, int,
-                                         const int64_t*, const int64_t*, const int*, cudaStream_t);
+                                         const int64_t*, const int64_t*, const int*, int, cudaStream_t);
 
 }  // namespace fe

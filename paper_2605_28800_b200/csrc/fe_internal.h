@@ -142,7 +142,8 @@ cudaError_t launch_xyfwd(const FftCtx& c, const T* P, void* ring, void* S2, int 
 bool zmul3_supported(int M, int nz);
 template <typename T>
 cudaError_t launch_zmul3(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
-                         int batch, const int64_t sstr[4], const int64_t kstr[4], const int perm[3], cudaStream_t st);
+                         int batch, const int64_t sstr[4], const int64_t kstr[4], const int perm[3],
+                         int variant /* 1: mirror pairs (k3_zmul), 2: merged edge phase (k5_zmul) */, cudaStream_t st);
 cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
 
 // ---- tensor (fe_tensor.cu) --------------------------------------------------------------------

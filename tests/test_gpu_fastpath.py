@@ -315,19 +315,22 @@ def test_paired_z_pass(fe, n, batch, dtype):
     g.precompute_tensor()
     P = g.state(P0)
     res = {}
-    for pairs in (1, 0):
-        g.set_option(fe.FE_OPT_Z_PAIRS, pairs)
-        res[pairs] = g.rhs(P, fi.TERM_ELEC).cpu().numpy().astype(np.float64)
+    for variant in (2, 1, 0):
+        g.set_option(fe.FE_OPT_Z_PAIRS, variant)
+        res[variant] = g.rhs(P, fi.TERM_ELEC).cpu().numpy().astype(np.float64)
     for b in range(batch):
         o = orc.Oracle(oracle_problem(w, b), elec="fft")
         want = o.rhs(P0[b], fi.TERM_ELEC)
-        assert rel_l2(res[1][b], want) < tol and rel_l2(res[0][b], want) < tol
-    assert rel_l2(res[1], res[0]) < (1e-13 if dtype == "f64" else 1e-5)
-    g.set_option(fe.FE_OPT_Z_PAIRS, 1)
-    Pa = g.state(P0)
-    g.step(Pa, w.dt, 12, fi.EULER, fi.TERM_ALL)
+        for variant in (2, 1, 0):
+            assert rel_l2(res[variant][b], want) < tol, (variant, b)
+    for variant in (2, 1):
+        assert rel_l2(res[variant], res[0]) < (1e-13 if dtype == "f64" else 1e-5), variant
     g.set_option(fe.FE_OPT_Z_PAIRS, 0)
     Pb = g.state(P0)
     g.step(Pb, w.dt, 12, fi.EULER, fi.TERM_ALL)
-    assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < (1e-12 if dtype == "f64" else 1e-4)
+    for variant in (2, 1):
+        g.set_option(fe.FE_OPT_Z_PAIRS, variant)
+        Pa = g.state(P0)
+        g.step(Pa, w.dt, 12, fi.EULER, fi.TERM_ALL)
+        assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < (1e-12 if dtype == "f64" else 1e-4), variant
     g.close()
