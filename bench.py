@@ -232,7 +232,6 @@ def run_cuda(args):
     rsz = 8 if args.dtype == "f64" else 4
     g = fe.Grid.from_workload(w, device=dev, dtype=args.dtype)
     g.set_option(fe.FE_OPT_FUSE_XY, args.fuse_xy)
-    g.set_option(fe.FE_OPT_Z_PAIRS, args.z_pairs)
     if args.xy_ring:
         g.set_option(fe.FE_OPT_XY_RING, args.xy_ring)
     t0 = time.time()
@@ -404,7 +403,7 @@ def run_cuda(args):
                 "config": {"workload": w.name, "grid": list(w.n), "batch": w.batch, "integrator": "euler",
                            "terms": "landau+gradient+elec+ext", "padded_fft": padded_dims(w),
                            "l2": "state and spectra exceed L2 (P 3N reals, spectra >= 4x that)",
-                           "parallelism": "replicas x%d" % world, "fuse_xy": args.fuse_xy, "z_pairs": args.z_pairs},
+                           "parallelism": "replicas x%d" % world, "fuse_xy": args.fuse_xy},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                 "clocks": cs.summary(), "cufft_baseline": cufft, "precompute_s": t_pre,
                 "energy_after": {"F_tot": float(en[4]), "finite": bool(np.isfinite(en).all())}}
@@ -562,7 +561,6 @@ def main():
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT comparison leg")
     ap.add_argument("--fuse-xy", type=int, default=0, choices=[0, 1],
                     help="FE_OPT_FUSE_XY: 1 = x and y passes fused through the L2 ring, 0 = separate kernels (default)")
-    ap.add_argument("--z-pairs", type=int, default=0, choices=[0, 1, 2], help="FE_OPT_Z_PAIRS")
     ap.add_argument("--xy-ring", type=int, default=0, help="FE_OPT_XY_RING (0 = automatic)")
     args = ap.parse_args()
     args.warmup_requested = args.warmup

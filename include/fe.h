@@ -114,12 +114,8 @@ fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map);
  *   FE_OPT_XY_TIMEOUTS read-only (fe_get_option synchronises the device): 1 if a wait inside the fused kernel ever
  *                      timed out (it cannot unless the device is shared with a kernel that never yields).
  *   FE_OPT_XY_RING     planes in the L2 ring of the fused pass; 0 (default) sizes it from the geometry (>= 24 planes,
- *                      <= 32 MB), 2..4096 fixes it (clamped to the number of planes).
- *   FE_OPT_Z_PAIRS     1: on a zero-padded z axis of transform length 256 the fused z pass works on mirror pairs of
- *                      tiles with one in-place exchange buffer, no staging buffer and K~ in registers (k3_zmul);
- *                      0 (default): one tile at a time with cp.async staging (k2_zmul), as on every other axis
- *                      length.  Measured on B200 at config 5a: 0.69 ms against 0.52 ms. */
-enum { FE_OPT_FUSE_XY = 0, FE_OPT_XY_TIMEOUTS = 1, FE_OPT_XY_RING = 2, FE_OPT_Z_PAIRS = 3 };
+ *                      <= 32 MB), 2..4096 fixes it (clamped to the number of planes). */
+enum { FE_OPT_FUSE_XY = 0, FE_OPT_XY_TIMEOUTS = 1, FE_OPT_XY_RING = 2 };
 fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value);
 fe_status fe_get_option(fe_grid* g, int32_t option, int32_t* value);
 

@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libfe_b200.so")
 PEAKS_LIB = os.path.join(HERE, "libfe_peaks.so")      # bench.py's harness kernels (csrc/bench_peaks.cu), not the product
-SOURCES = ["fe_api.cu", "fe_fft.cu", "fe_fft2_x.cu", "fe_fft2_axis.cu", "fe_fft2_z.cu", "fe_fft2_xy.cu", "fe_fft2_z3.cu", "fe_tensor.cu", "fe_local.cu", "fe_integ.cu"]
+SOURCES = ["fe_api.cu", "fe_fft.cu", "fe_fft2_x.cu", "fe_fft2_axis.cu", "fe_fft2_z.cu", "fe_fft2_xy.cu", "fe_tensor.cu", "fe_local.cu", "fe_integ.cu"]
 HEADERS = [os.path.join(CSRC, "fe_internal.h"), os.path.join(CSRC, "fe_fft2.cuh"), os.path.join(ROOT, "include", "fe.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

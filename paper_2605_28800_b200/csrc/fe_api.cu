@@ -61,7 +61,6 @@ struct fe_grid {
     size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_K[6], o_part, o_cnt, o_box, o_Sbox, total_bytes;
     int opt_fuse_xy;                 // FE_OPT_FUSE_XY
     int opt_xy_ring;                 // FE_OPT_XY_RING (0: automatic)
-    int opt_z_pairs;                 // FE_OPT_Z_PAIRS
     int nblk;
     bool tensor_ready;
     bool fast[3];                    // size-specialised register FFT kernels available for the x / y / z pass
@@ -246,7 +245,6 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     g->mixed = 0;
     g->opt_fuse_xy = 0;
     g->opt_xy_ring = 0;
-    g->opt_z_pairs = 0;
     g->map = nullptr;
     g->ws = nullptr;
     g->ws_bytes = 0;
@@ -465,11 +463,6 @@ extern "C" fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value)
         g->gvalid = false;               // a captured graph holds the other kernels
         return FE_OK;
     }
-    if (option == FE_OPT_Z_PAIRS && value >= 0 && value <= 2) {
-        g->opt_z_pairs = value;
-        g->gvalid = false;
-        return FE_OK;
-    }
     if (option == FE_OPT_XY_RING && value >= 0 && value <= 4096) {
         g->opt_xy_ring = value;
         g->gvalid = false;
@@ -483,7 +476,6 @@ extern "C" fe_status fe_get_option(fe_grid* g, int32_t option, int32_t* value)
     if (!g || !value) return fail(FE_EINVAL, "null argument");
     if (option == FE_OPT_FUSE_XY) { *value = g->opt_fuse_xy; return FE_OK; }
     if (option == FE_OPT_XY_RING) { *value = g->opt_xy_ring; return FE_OK; }
-    if (option == FE_OPT_Z_PAIRS) { *value = g->opt_z_pairs; return FE_OK; }
     if (option == FE_OPT_XY_TIMEOUTS) {
         *value = 0;
         if (!g->ws) return FE_OK;
@@ -651,9 +643,7 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     g->launches += 2;
     }
     mark(g, K_ZMUL, st);
-    if (g->fast[2] && g->opt_z_pairs && zmul3_supported(q.m[2], nz))
-        FE_CUDA(launch_zmul3<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, g->opt_z_pairs, st));
-    else if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, st));
+    if (g->fast[2]) FE_CUDA(launch_zmul2<T>(g->ctx, S2, Kt, g->d_members, nz, My, G, B, zs, ks, perm, st));
     else FE_CUDA(launch_zmul<T>(g->ctx, S2, Kt, g->d_members, q.n[2], q.m[1], q.lanes, q.pitch, B, st));
     mark(g, K_YINV, st);
     if (g->fast[1]) {

@@ -138,12 +138,6 @@ bool xy_supported(int Mx, int My, int nx, int ny);
 template <typename T>
 cudaError_t launch_xyfwd(const FftCtx& c, const T* P, void* ring, void* S2, int nx, int ny, int nz, int nplanes, int G,
                          int ring_slots, int64_t s2_sz, int64_t s2_sg, int64_t s2_sb, int* counters, cudaStream_t st);
-// fused z pass on mirror pairs of tiles (fe_fft2_z3.cu): zero-padded 256-point axis only
-bool zmul3_supported(int M, int nz);
-template <typename T>
-cudaError_t launch_zmul3(const FftCtx& c, void* S, const T* Kt, const DevMember* members, int nz, int My, int ngroups,
-                         int batch, const int64_t sstr[4], const int64_t kstr[4], const int perm[3],
-                         int variant /* 1: mirror pairs (k3_zmul), 2: merged edge phase (k5_zmul) */, cudaStream_t st);
 cudaError_t fft_configure();     // raise dynamic shared memory limits; call once
 
 // ---- tensor (fe_tensor.cu) --------------------------------------------------------------------

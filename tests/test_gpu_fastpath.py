@@ -297,40 +297,3 @@ def test_fused_xy_pass_through_the_l2_ring(fe, n, batch, dtype):
     assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < (1e-12 if dtype == "f64" else 1e-4)
     assert g.get_option(fe.FE_OPT_XY_TIMEOUTS) == 0
     g.close()
-
-
-@pytest.mark.parametrize("n,batch,dtype", [
-    ((64, 128, 128), 2, "f64"),        # z 256p; y 256p in slot order; two members
-    ((64, 32, 128), 1, "f64"),         # z 256p; y 64 (natural ky order, register-I/O y pass)
-    ((64, 128, 70), 1, "f64"),         # z 256p with 70 data rows (partial pruning)
-    ((64, 128, 128), 1, "f32"),
-])
-def test_paired_z_pass(fe, n, batch, dtype):
-    """FE_OPT_Z_PAIRS: the fused z pass on mirror pairs of tiles (k3_zmul) against oracle-FFT, against the one-tile
-    kernel it replaces on the zero-padded 256-point axis, per member, and over steps."""
-    w = _workload(n, batch=batch)
-    tol = TOL_RHS64 if dtype == "f64" else TOL32
-    P0 = w.P0 if dtype == "f64" else w.P0.astype(np.float32).astype(np.float64)
-    g = fe.Grid.from_workload(w, dtype=dtype)
-    g.precompute_tensor()
-    P = g.state(P0)
-    res = {}
-    for variant in (2, 1, 0):
-        g.set_option(fe.FE_OPT_Z_PAIRS, variant)
-        res[variant] = g.rhs(P, fi.TERM_ELEC).cpu().numpy().astype(np.float64)
-    for b in range(batch):
-        o = orc.Oracle(oracle_problem(w, b), elec="fft")
-        want = o.rhs(P0[b], fi.TERM_ELEC)
-        for variant in (2, 1, 0):
-            assert rel_l2(res[variant][b], want) < tol, (variant, b)
-    for variant in (2, 1):
-        assert rel_l2(res[variant], res[0]) < (1e-13 if dtype == "f64" else 1e-5), variant
-    g.set_option(fe.FE_OPT_Z_PAIRS, 0)
-    Pb = g.state(P0)
-    g.step(Pb, w.dt, 12, fi.EULER, fi.TERM_ALL)
-    for variant in (2, 1):
-        g.set_option(fe.FE_OPT_Z_PAIRS, variant)
-        Pa = g.state(P0)
-        g.step(Pa, w.dt, 12, fi.EULER, fi.TERM_ALL)
-        assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < (1e-12 if dtype == "f64" else 1e-4), variant
-    g.close()
