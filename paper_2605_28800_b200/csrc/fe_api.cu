@@ -663,9 +663,18 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
     return FE_OK;
 }
 
+// folded stage combination of the multistep / embedded integrators (LocalArgs::kOut, lk, lc)
+struct StageLin {
+    void* kOut = nullptr;
+    const void* lk[4] = {nullptr, nullptr, nullptr, nullptr};
+    double lc[4] = {0, 0, 0, 0};
+    int nlin = 0;
+    void add(const void* k, double c) { if (c != 0.0) { lk[nlin] = k; lc[nlin] = c; ++nlin; } }
+};
+
 template <typename T>
 static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double cy, const T* accIn, T* accOut, double ca,
-                       uint32_t terms, cudaStream_t st)
+                       uint32_t terms, cudaStream_t st, const StageLin* lin = nullptr)
 {
     const bool elec = (terms & FE_TERM_ELEC) != 0;
     if (elec) {
@@ -682,6 +691,11 @@ static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double c
     a.accOut = accOut;
     a.cy = cy;
     a.ca = ca;
+    if (lin) {
+        a.kOut = lin->kOut;
+        a.nlin = lin->nlin;
+        for (int j = 0; j < lin->nlin; ++j) { a.lk[j] = lin->lk[j]; a.lc[j] = lin->lc[j]; }
+    }
     a.map = g->map;
     a.mats = g->d_mats;
     a.members = g->d_members;
@@ -757,30 +771,24 @@ static fe_status step_T(fe_grid* g, T* P, double dt, int nsteps, int integ, uint
         // P <- P + dt/2 (f_n + f(P*)); the history restarts with every call
         T* F[3] = {reinterpret_cast<T*>(g->ws + g->o_K[0]), reinterpret_cast<T*>(g->ws + g->o_K[1]),
                    reinterpret_cast<T*>(g->ws + g->o_K[2])};
-        T* FS = reinterpret_cast<T*>(g->ws + g->o_K[3]);
-        const int64_t n = (int64_t)g->desc.batch * 3 * g->N;
         for (int i = 0; i < nsteps; ++i) {
+            // both stage combinations ride on the local step's epilogue (no separate streaming passes):
+            //   f_n = f(P) -> F[0],  P* = P + [c1 f_{n-1} + c2 f_{n-2}] + c0 f_n -> Y;   P <- P + dt/2 f_n + dt/2 f(P*)
             const double tn = t0 + i * dt;
             g->tstage = tn;
-            if ((s = stage<T>(g, P, nullptr, F[0], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
-            LinArgs a;
-            memset(&a, 0, sizeof(a));
-            if (i < 2) {
-                a.k[0] = F[0]; a.c[0] = dt;
-                FE_CUDA(launch_lincomb<T>(Y, P, a, 1, n, st));
-            } else {
-                a.k[0] = F[0]; a.c[0] = dt * 23.0 / 12.0;
-                a.k[1] = F[1]; a.c[1] = -dt * 16.0 / 12.0;
-                a.k[2] = F[2]; a.c[2] = dt * 5.0 / 12.0;
-                FE_CUDA(launch_lincomb<T>(Y, P, a, 3, n, st));
+            StageLin pre;
+            pre.kOut = F[0];
+            double c0 = dt;
+            if (i >= 2) {
+                c0 = dt * 23.0 / 12.0;
+                pre.add(F[1], -dt * 16.0 / 12.0);
+                pre.add(F[2], dt * 5.0 / 12.0);
             }
+            if ((s = stage<T>(g, P, P, Y, c0, nullptr, nullptr, 0.0, terms, st, &pre)) != FE_OK) return s;
             g->tstage = tn + dt;
-            if ((s = stage<T>(g, Y, nullptr, FS, 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
-            memset(&a, 0, sizeof(a));
-            a.k[0] = F[0]; a.c[0] = 0.5 * dt;
-            a.k[1] = FS;   a.c[1] = 0.5 * dt;
-            FE_CUDA(launch_lincomb<T>(P, P, a, 2, n, st));
-            g->launches += 2;
+            StageLin cor;
+            cor.add(F[0], 0.5 * dt);
+            if ((s = stage<T>(g, Y, P, P, 0.5 * dt, nullptr, nullptr, 0.0, terms, st, &cor)) != FE_OK) return s;
             T* t = F[2]; F[2] = F[1]; F[1] = F[0]; F[0] = t;
         }
     } else {
@@ -896,20 +904,20 @@ static fe_status rk45_T(fe_grid* g, T* P, double t_span, double dt_init, double 
     fe_status s;
     while (t < t_span && acc + rej < max_steps) {
         const double h = dt < t_span - t ? dt : t_span - t;
+        // stage i evaluates K[i] = f(Y_i) and, in the same epilogue, forms Y_{i+1} = P + h sum_{j <= i} a_{i+1,j} K[j]
+        // (terms in ascending j, the stage's own k last); the stage states alternate between two buffers
+        T* Yab[2] = {Y, reinterpret_cast<T*>(g->ws + g->o_ACC)};
         for (int i = 0; i < 6; ++i) {
-            const T* Yi = P;
-            if (i > 0) {
-                LinArgs a;
-                memset(&a, 0, sizeof(a));
-                int nk = 0;
-                for (int j = 0; j < i; ++j)
-                    if (A[i][j] != 0.0) { a.k[nk] = K[j]; a.c[nk] = h * A[i][j]; ++nk; }
-                FE_CUDA(launch_lincomb<T>(Y, P, a, nk, n, st));
-                g->launches += 1;
-                Yi = Y;
-            }
+            const T* Yi = i == 0 ? P : Yab[(i - 1) & 1];
             g->tstage = time0 + t + C[i] * h;
-            if ((s = stage<T>(g, Yi, nullptr, K[i], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+            if (i < 5) {
+                StageLin lin;
+                lin.kOut = K[i];
+                for (int j = 0; j < i; ++j) lin.add(K[j], h * A[i + 1][j]);
+                if ((s = stage<T>(g, Yi, P, Yab[i & 1], h * A[i + 1][i], nullptr, nullptr, 0.0, terms, st, &lin)) != FE_OK) return s;
+            } else {
+                if ((s = stage<T>(g, Yi, nullptr, K[i], 1.0, nullptr, nullptr, 0.0, terms, st)) != FE_OK) return s;
+            }
         }
         evals += 6;
         LinArgs b5, d;

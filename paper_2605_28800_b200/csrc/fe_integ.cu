@@ -1,21 +1,10 @@
-// fe_integ.cu -- array kernels of the multistep / adaptive integrators:
-//   k_lincomb     out = base + sum_j c_j k_j                      (stage states of RK45, predictor / corrector of AB3M2)
+// fe_integ.cu -- array kernel of the adaptive integrator:
 //   k_rk45_final  y5 = P + sum_j b5_j k_j,  err = max |sum_j d_j k_j|   (Cash-Karp 5th-order solution + embedded error)
-// Plain streaming passes (HBM bound); the right-hand sides themselves come from the fused local step (fe_local.cu).
+// A plain streaming pass (HBM bound).  The right-hand sides and every other stage combination of RK45 and AB3M2 come
+// from the fused local step's epilogue (fe_local.cu: LocalArgs::kOut / lk / lc).
 #include "fe_internal.h"
 
 namespace fe {
-
-template <typename T, int NK>
-__global__ void __launch_bounds__(256) k_lincomb(T* out, const T* base, LinArgs a, int64_t n)   // out may alias base
-{
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-        T v = base[i];
-#pragma unroll
-        for (int j = 0; j < NK; ++j) v = v + (T)a.c[j] * static_cast<const T*>(a.k[j])[i];
-        out[i] = v;
-    }
-}
 
 // max that keeps a NaN once it has seen one (fmax would return the other operand and hide a blown-up cell)
 __device__ __forceinline__ double nanmax(double m, double v) { return (v > m || v != v) ? v : m; }
@@ -50,21 +39,6 @@ __global__ void __launch_bounds__(256) k_rk45_final(T* __restrict__ y5, const T*
 }
 
 template <typename T>
-cudaError_t launch_lincomb(T* out, const T* base, const LinArgs& a, int nk, int64_t n, cudaStream_t st)
-{
-    const int grid = (int)((n + 255) / 256 < 148 * 16 ? (n + 255) / 256 : 148 * 16);
-    switch (nk) {
-        case 1: k_lincomb<T, 1><<<grid, 256, 0, st>>>(out, base, a, n); break;
-        case 2: k_lincomb<T, 2><<<grid, 256, 0, st>>>(out, base, a, n); break;
-        case 3: k_lincomb<T, 3><<<grid, 256, 0, st>>>(out, base, a, n); break;
-        case 4: k_lincomb<T, 4><<<grid, 256, 0, st>>>(out, base, a, n); break;
-        case 5: k_lincomb<T, 5><<<grid, 256, 0, st>>>(out, base, a, n); break;
-        default: return cudaErrorInvalidValue;
-    }
-    return cudaGetLastError();
-}
-
-template <typename T>
 cudaError_t launch_rk45_final(T* y5, const T* P, const LinArgs& b5, const LinArgs& d, int64_t n, double* err, cudaStream_t st)
 {
     cudaError_t e = cudaMemsetAsync(err, 0, sizeof(double), st);
@@ -74,8 +48,6 @@ cudaError_t launch_rk45_final(T* y5, const T* P, const LinArgs& b5, const LinArg
     return cudaGetLastError();
 }
 
-template cudaError_t launch_lincomb<double>(double*, const double*, const LinArgs&, int, int64_t, cudaStream_t);
-template cudaError_t launch_lincomb<float>(float*, const float*, const LinArgs&, int, int64_t, cudaStream_t);
 template cudaError_t launch_rk45_final<double>(double*, const double*, const LinArgs&, const LinArgs&, int64_t, double*, cudaStream_t);
 template cudaError_t launch_rk45_final<float>(float*, const float*, const LinArgs&, const LinArgs&, int64_t, double*, cudaStream_t);
 

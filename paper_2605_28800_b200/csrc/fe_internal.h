@@ -157,6 +157,12 @@ struct LocalArgs {
     const void* accIn;    // accOut = accIn + ca * k (both null: skipped)
     void* accOut;
     double cy, ca;
+    // stage combinations of the multistep / embedded integrators folded into the same epilogue:
+    //   kOut = k (raw right-hand side, may be null);  Yout = baseY + sum_{j < nlin} lc[j] * lk[j] + cy * k
+    void* kOut;
+    const void* lk[4];
+    double lc[4];
+    int nlin;
     const uint8_t* map;   // null: material 0 everywhere
     const DevLandau* mats;    // [B][nmat]
     const DevMember* members; // [B]
@@ -199,9 +205,6 @@ struct LinArgs {
     const void* k[6];
     double c[6];
 };
-// out = base + sum_{j < nk} c_j k_j   (nk in 1..5; out may alias base)
-template <typename T>
-cudaError_t launch_lincomb(T* out, const T* base, const LinArgs& a, int nk, int64_t n, cudaStream_t st);
 // y5 = P + sum_j b5.c_j k_j;  *err (device double, reset here) = max_i |sum_j d.c_j k_j[i]|
 template <typename T>
 cudaError_t launch_rk45_final(T* y5, const T* P, const LinArgs& b5, const LinArgs& d, int64_t n, double* err, cudaStream_t st);

@@ -295,6 +295,17 @@ __global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
                 bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r];
             }
         }
+        if (a.kOut) {
+            T* ko = static_cast<T*>(a.kOut) + (int64_t)b * 3 * N;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) ko[i * N + r] = k[i];
+        }
+        for (int j = 0; j < a.nlin; ++j) {
+            const T* lkj = static_cast<const T*>(a.lk[j]) + (int64_t)b * 3 * N;
+            const T cj = (T)a.lc[j];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) bv[i] = bv[i] + cj * lkj[i * N + r];
+        }
 #pragma unroll
         for (int i = 0; i < 3; ++i) Yout[i * N + r] = bv[i] + cy * k[i];
         if (ao) {
@@ -610,6 +621,11 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
             if (actA) kA[i] = L * EA[i];
             if (actB) kB[i] = L * EB[i];
         }
+        if (a.kOut) {
+            T* ko = static_cast<T*>(a.kOut) + (int64_t)b * 3 * N;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) *reinterpret_cast<P2*>(ko + i * N + r) = P2{kA[i], kB[i]};
+        }
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             P2 bv = {0, 0};
@@ -617,6 +633,11 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
                 // Euler: the stage base is the state itself, already in the tile (vacuum cells hold their raw value in memory)
                 if (base_is_Y && actA && actB) bv = pc[i];
                 else bv = ldp(base + i * N + r);
+            }
+            for (int j = 0; j < a.nlin; ++j) {
+                const P2 lv = ldp(static_cast<const T*>(a.lk[j]) + (int64_t)b * 3 * N + i * N + r);
+                const T cj = (T)a.lc[j];
+                bv = P2{bv.a + cj * lv.a, bv.b + cj * lv.b};
             }
             *reinterpret_cast<P2*>(Yout + i * N + r) = P2{bv.a + cy * kA[i], bv.b + cy * kB[i]};
             if (ao) {
