@@ -7,6 +7,8 @@
 //            zero outside the sample / in vacuum cells, c_ia = G11 (a == i) or G44 + G44', Gm = G12 + G44 - G44'
 //   then the integrator stage:  Yout = baseY + cy * k,  accOut = accIn + ca * k
 #include "fe_internal.h"
+#include <string.h>
+#include <cuda.h>          // CUtensorMap and cuTensorMapEncodeTiled's signature only; the entry point is fetched at run time
 
 namespace fe {
 
@@ -335,17 +337,64 @@ template <int BYTES> __device__ __forceinline__ void cp_async_zfill(void* smem, 
     asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;\n" ::"r"(s), "l"(gmem), "n"(BYTES), "r"(src_bytes));
 }
 
-template <typename T, bool MAP, bool MIXED>
-__global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
+// mbarrier / tensor-copy helpers of the TMA halo loader
+__device__ __forceinline__ unsigned lsm_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void l_mbar_init(void* bar, int count)
 {
-    extern __shared__ __align__(16) unsigned char lsm[];
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(lsm_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void l_mbar_expect_tx(void* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(lsm_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void l_mbar_wait(void* bar, unsigned parity)
+{
+    const unsigned addr = lsm_u32(bar);
+    unsigned done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+// 4-D box (x, y, z, component) of the state -> shared memory; coordinates outside the tensor read as zero
+__device__ __forceinline__ void l_tma_load_4d(void* smem_dst, const CUtensorMap* map, int cx0, int cy0, int cz0, int cc0, void* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];\n" ::"r"(
+            lsm_u32(smem_dst)),
+        "l"(map), "r"(cx0), "r"(cy0), "r"(cz0), "r"(cc0), "r"(lsm_u32(bar))
+        : "memory");
+}
+
+// bytes of one plane slot of k_local2 (three components of a 68 x 10 tile), rounded up to the 128-byte alignment of a
+// tensor copy's destination
+template <typename T> __host__ __device__ constexpr size_t k2_slot_bytes() { return ((size_t)3 * k2Tile * sizeof(T) + 127) / 128 * 128; }
+
+// TMA = true (no material map, no periodic axis): a plane of the halo tile arrives as ONE tensor copy
+// (cp.async.bulk.tensor, box 68 x 10 x 1 x 3 components starting at (x0 - 2, y0 - 1, z); cells outside the sample are
+// zero-filled by the copy engine) issued by one thread and completed on an mbarrier, instead of four cp.async per thread.
+template <typename T, bool MAP, bool MIXED, bool TMA = false>
+__global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_constant__ CUtensorMap tmap)
+{
+    extern __shared__ __align__(128) unsigned char lsm[];
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
     // three planes ahead of their use; with a map the loader goes through registers (vacuum cells are zeroed).
     constexpr int NS = MAP ? 4 : 5;
-    T* tiles = reinterpret_cast<T*>(lsm);                                   // [NS][3][k2Tile]
-    unsigned char* flags = lsm + (size_t)NS * 3 * k2Tile * sizeof(T);       // [NS][k2Tile]
+    constexpr int SLOT = (int)(k2_slot_bytes<T>() / sizeof(T));             // elements between two plane slots
+    static_assert(!(TMA && MAP), "the tensor-copy loader has no vacuum masking");
+    T* tiles = reinterpret_cast<T*>(lsm);                                   // [NS][SLOT >= 3 k2Tile]
+    unsigned char* flags = lsm + (size_t)NS * SLOT * sizeof(T);             // [NS][k2Tile]
     LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + NS * k2Tile);  // [nmat]
     unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(
+        lsm + (((size_t)(sact + a.nmat - lsm) + 7) / 8) * 8);                // [NS] mbarriers of the tensor-copy loader
     using P2 = pair_t<T>;
 
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
@@ -435,7 +484,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
         bool zin = true;
         if (zz < 0 || zz >= nz) { if (a.periodic[2]) zz = ((zz % nz) + nz) % nz; else zin = false; }
         const int64_t r0 = (int64_t)zz * nxy;
-        T* tl = tiles + slot_of(z) * 3 * k2Tile;
+        T* tl = tiles + slot_of(z) * SLOT;
 #pragma unroll
         for (int k = 0; k < k2NL; ++k) {
             if (l_so[k] < 0) continue;
@@ -448,7 +497,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
     };
     auto store_plane = [&](int z) {
         const int slot = slot_of(z);
-        T* tl = tiles + slot * 3 * k2Tile;
+        T* tl = tiles + slot * SLOT;
         unsigned char* fl = flags + slot * k2Tile;
 #pragma unroll
         for (int k = 0; k < k2NL; ++k) {
@@ -462,13 +511,32 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
             }
         }
     };
-    __syncthreads();          // coefficient tables visible (fetch_plane reads sact)
+    // tensor-copy loader: plane z of all three components in one copy, completion on the slot's mbarrier
+    auto tma_plane = [&](int z) {
+        if (z > z1 || t != 0) return;
+        const int slot = slot_of(z);
+        l_mbar_expect_tx(&bars[slot], (unsigned)(3 * k2Tile * sizeof(T)));
+        l_tma_load_4d(tiles + slot * SLOT, &tmap, x0 - 2, y0 - 1, z, 3 * b, &bars[slot]);
+    };
+    auto tma_wait = [&](int z) { l_mbar_wait(&bars[slot_of(z)], (unsigned)(((z - z0 + 1) / NS) & 1)); };
+    if (TMA && t == 0) {
+        for (int i = 0; i < NS; ++i) l_mbar_init(&bars[i], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();          // coefficient tables visible (fetch_plane reads sact); mbarriers initialised
     if (MAP) {
         fetch_plane(z0 - 1);
         store_plane(z0 - 1);
         fetch_plane(z0);
         store_plane(z0);
         fetch_plane(z0 + 1);
+    } else if (TMA) {
+        tma_plane(z0 - 1);
+        tma_plane(z0);
+        tma_plane(z0 + 1);
+        tma_plane(z0 + 2);
+        tma_wait(z0 - 1);         // the loop waits for plane z + 1 only: the first two are awaited here
+        tma_wait(z0);
     } else {
         async_plane(z0 - 1);
         async_plane(z0);
@@ -509,6 +577,10 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
             store_plane(z + 1);
             __syncthreads();
             if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
+        } else if (TMA) {
+            tma_wait(z + 1);                                 // planes <= z+1 have landed
+            __syncthreads();                                 // every thread is done with plane z-2
+            tma_plane(z + 3);                                // into the slot of plane z-2
         } else {
             asm volatile("cp.async.wait_group 1;\n" ::);     // planes <= z+1 have landed
             __syncthreads();
@@ -522,9 +594,9 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
             for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + rn);
         }
         const int sm1 = slot_of(z - 1), s00 = slot_of(z), sp1 = slot_of(z + 1);
-        const T* m0 = tiles + sm1 * 3 * k2Tile;     // plane z-1
-        const T* c = tiles + s00 * 3 * k2Tile;      // plane z
-        const T* p1 = tiles + sp1 * 3 * k2Tile;     // plane z+1
+        const T* m0 = tiles + sm1 * SLOT;           // plane z-1
+        const T* c = tiles + s00 * SLOT;            // plane z
+        const T* p1 = tiles + sp1 * SLOT;           // plane z+1
         const unsigned char* fm = flags + sm1 * k2Tile;
         const unsigned char* fc = flags + s00 * k2Tile;
         const unsigned char* fp = flags + sp1 * k2Tile;
@@ -649,6 +721,41 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a)
 
 }
 
+// Tensor map of a state array [B * 3][nz][ny][nx] with the 68 x 10 x 1 x 3 box of k_local2's plane slots.  The encoder is
+// a driver entry point fetched at run time (no link against libcuda).  Returns false when the geometry does not meet the
+// copy engine's rules (row pitch a multiple of 16 bytes) or the entry point is missing: the caller uses cp.async then.
+template <typename T> static bool make_state_map(const LocalArgs& a, CUtensorMap* out)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn enc = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            enc = reinterpret_cast<encode_fn>(fn);
+        tried = true;
+    }
+    if (!enc) return false;
+    // fp64 only: the box starts two cells left of the tile (x0 - 2), 16 bytes in fp64 but 8 in fp32, and the copy engine
+    // raised an illegal-instruction fault on the 8-byte-aligned start on B200; fp32 keeps the cp.async loader
+    if (sizeof(T) != 8) return false;
+    const cuuint64_t nx = a.n[0], ny = a.n[1], nz = a.n[2];
+    if ((nx * sizeof(T)) % 16 || nx < (cuuint64_t)k2PX || ny < (cuuint64_t)k2HY) return false;
+    if (reinterpret_cast<uintptr_t>(a.Y) % 16) return false;
+    const cuuint64_t dims[4] = {nx, ny, nz, (cuuint64_t)3 * a.batch};
+    const cuuint64_t strides[3] = {nx * sizeof(T), nx * ny * sizeof(T), nx * ny * nz * sizeof(T)};
+    const cuuint32_t box[4] = {(cuuint32_t)k2PX, (cuuint32_t)k2HY, 1, 3};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    const CUresult r = enc(out, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
+                           const_cast<void*>(a.Y), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
 template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t st)
 {
     LocalArgs a = a0;
@@ -664,8 +771,12 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     a.zchunk = zc;
     dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
     const int ns = a.map ? 4 : 5;         // ring slots of k_local2
-    const size_t smem = two ? (size_t)ns * 3 * k2Tile * sizeof(T) + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1)
+    const size_t smem = two ? (size_t)ns * k2_slot_bytes<T>() + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1) + 8 + ns * 8
                             : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
+    // halo planes by tensor copy (zero fill outside the sample) when there is neither a material map nor a periodic axis
+    CUtensorMap tmap;
+    memset(&tmap, 0, sizeof(tmap));
+    const bool tma = two && !a.map && !(a.periodic[0] | a.periodic[1] | a.periodic[2]) && make_state_map<T>(a, &tmap);
     static PerDevice<int> cache;
     int& configured = cache.here();
     if (!configured) {
@@ -679,16 +790,21 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e != cudaSuccess) return e;
         configured = 1;
     }
     if (two) {
         if (a.map) {
-            if (a.mixed) k_local2<T, true, true><<<grid, 256, smem, st>>>(a);
-            else k_local2<T, true, false><<<grid, 256, smem, st>>>(a);
+            if (a.mixed) k_local2<T, true, true><<<grid, 256, smem, st>>>(a, tmap);
+            else k_local2<T, true, false><<<grid, 256, smem, st>>>(a, tmap);
+        } else if (tma) {
+            if (a.mixed) k_local2<T, false, true, true><<<grid, 256, smem, st>>>(a, tmap);
+            else k_local2<T, false, false, true><<<grid, 256, smem, st>>>(a, tmap);
         } else {
-            if (a.mixed) k_local2<T, false, true><<<grid, 256, smem, st>>>(a);
-            else k_local2<T, false, false><<<grid, 256, smem, st>>>(a);
+            if (a.mixed) k_local2<T, false, true><<<grid, 256, smem, st>>>(a, tmap);
+            else k_local2<T, false, false><<<grid, 256, smem, st>>>(a, tmap);
         }
         return cudaGetLastError();
     }
