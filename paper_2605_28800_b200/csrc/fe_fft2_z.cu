@@ -15,9 +15,46 @@
 // Both inter-step twiddles w_M^{+-n2 k1} are applied by the thread that owns k1: it loads its R2 - 1 factors once
 // per tile and uses them for the three components in both directions (the R1-point steps move no twiddles).
 #include "fe_fft2.cuh"
+#include <string.h>
+#include <cuda.h>          // CUtensorMap and cuTensorMapEncodeTiled's signature only; the entry point is fetched at run time
 
 namespace fe {
 namespace v2 {
+
+// ---- tensor-copy (TMA) staging of the tiled layouts: one copy per tile / per K~ tile, completion on an mbarrier ----------
+__device__ __forceinline__ unsigned z_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void z_mbar_init(void* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(z_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void z_mbar_expect_tx(void* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(z_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void z_mbar_wait(void* bar, unsigned parity)
+{
+    const unsigned addr = z_smem_u32(bar);
+    unsigned done;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(done)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void z_tma_load_5d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, int c4, void* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];\n" ::"r"(
+            z_smem_u32(smem_dst)),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(z_smem_u32(bar))
+        : "memory");
+}
 
 // factorisation used by the fused pass: R2 frequencies per thread (3 components in registers)
 template <int M> struct ZFact;
@@ -83,7 +120,7 @@ template <typename T, int M, int LANES, bool PRUNE> struct ZCfg {
     static constexpr size_t ex_bytes = (size_t)3 * TILE * sizeof(cx<T>);
     static constexpr size_t st_bytes = (size_t)3 * NIN * LANES * sizeof(cx<T>);
     static constexpr size_t k_bytes = ((size_t)6 * HZ * LANES * sizeof(T) + 15) / 16 * 16;
-    static constexpr size_t smem = tw_bytes + ex_bytes + st_bytes + k_bytes;
+    static constexpr size_t smem = tw_bytes + ex_bytes + st_bytes + k_bytes + 16;       // + two mbarriers (TMA staging)
 };
 
 // position of a block in its sequence of tiles; advanced without divisions (the loop head is executed by every
@@ -117,9 +154,13 @@ struct ZIter {
     __device__ __forceinline__ int ky(const Z2Args& a) const { return m ? a.My - kyh : kyh; }
 };
 
-template <typename T, int M, int LANES, bool PRUNE>
+// TMA = true (tiled layouts): the rows of a tile (box LANES x 1 ky x NIN rows x 1 kx group x 3 components of S) and the
+// K~ tile of an item (box LANES x HZ x 1 x 1 x 6 of Kt) each arrive as ONE tensor copy issued by thread 0 and completed on
+// an mbarrier, instead of 12 + 9 cp.async per thread and tile; rows beyond nz are zero-filled by the copy engine.
+template <typename T, int M, int LANES, bool PRUNE, bool TMA = false>
 __global__ void __launch_bounds__(ZCfg<T, M, LANES, PRUNE>::THREADS, ZCfg<T, M, LANES, PRUNE>::THREADS <= 64 ? 4 : (ZCfg<T, M, LANES, PRUNE>::smem > 112 * 1024 ? 1 : 2))
-k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
+k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a, const __grid_constant__ CUtensorMap smap,
+        const __grid_constant__ CUtensorMap kmap)
 {
     using C = ZCfg<T, M, LANES, PRUNE>;
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, NT1 = C::NT1, TILE = C::TILE, NIN = C::NIN, HZ = C::HZ;
@@ -128,6 +169,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     cx<T>* buf = tw + M;                                            // exchange [3][M][LANES]
     cx<T>* stage = buf + 3 * TILE;                                  // staged input [3][NIN][LANES]
     T* kbuf = reinterpret_cast<T*>(stage + 3 * NIN * LANES);        // K~ tile [6][HZ][LANES]
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(kbuf) + C::k_bytes);  // [2]
     const int lane = threadIdx.x % LANES, tp = threadIdx.x / LANES;
     const int64_t sa = a.s_z, cs = a.cs, kcs = a.kcs;
 
@@ -187,15 +229,41 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     cur.set_item(blockIdx.x % a.ngroups, blockIdx.x / a.ngroups, a);
     if (!cur.valid(a)) return;
     const int dq = gridDim.x / a.ngroups, dr = gridDim.x % a.ngroups;
-    if (PRUNE && a.nz < NIN) {              // padding rows inside the staged half: cleared once, never written again
+    // tensor-copy staging: thread 0 issues, everybody waits on the mbarriers (bars[0]: tile rows, bars[1]: K~ tile)
+    auto tma_tile = [&](const ZIter& it) {
+        const int ky = it.ky(a);
+        int slot = ky;
+        if (a.la >= 0)
+            slot = ((ky & ((1 << a.la) - 1)) << (a.lb + a.lc)) | (((ky >> a.la) & ((1 << a.lb) - 1)) << a.lc) |
+                   (ky >> (a.la + a.lb));
+        z_mbar_expect_tx(&bars[0], (unsigned)(3 * NIN * LANES * sizeof(cx<T>)));
+        z_tma_load_5d(stage, &smap, 0, slot, 0, it.kxg, 3 * it.b, &bars[0]);
+    };
+    auto tma_k = [&](const ZIter& it) {
+        z_mbar_expect_tx(&bars[1], (unsigned)(6 * HZ * LANES * sizeof(T)));
+        z_tma_load_5d(kbuf, &kmap, 0, 0, it.kyh, it.kxg, 0, &bars[1]);
+    };
+    unsigned sphase = 0, kphase = 0;
+    bool kpend = true;
+    if (!TMA && PRUNE && a.nz < NIN) {      // padding rows inside the staged half: cleared once, never written again
         for (int e = threadIdx.x; e < 3 * NIN * LANES; e += C::THREADS) stage[e] = cx<T>{0, 0};
         __syncthreads();
     }
     cx<T>* cur_base = tile_base(cur);       // carried from the prefetch of a tile to its turn in the loop
-    prefetch_tile(cur_base);
-    cp_async_commit();                      // group A: input of the first tile
-    prefetch_k(cur, ic_all{}, ic_zero{});
-    cp_async_commit();                      // group B: K~ of the first item
+    if (TMA) {
+        if (threadIdx.x == 0) {
+            z_mbar_init(&bars[0], 1);
+            z_mbar_init(&bars[1], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+            tma_tile(cur);
+            tma_k(cur);
+        }
+    } else {
+        prefetch_tile(cur_base);
+        cp_async_commit();                  // group A: input of the first tile
+        prefetch_k(cur, ic_all{}, ic_zero{});
+        cp_async_commit();                  // group B: K~ of the first item
+    }
     load_twiddles<T, M>(tw, static_cast<const cx<T>*>(a.tw), threadIdx.x, C::THREADS);
 
     while (cur.valid(a)) {
@@ -204,8 +272,14 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         const double escale = a.members[cur.b].escale;  // issued here, consumed after the forward transform
         ZIter nxt = cur;
         nxt.next(a, dq, dr);
-        cp_async_wait<1>();                 // this tile's input has landed (the newest group may still be in flight)
-        __syncthreads();                    // ... for every thread; also: previous tile's exchange reads are done
+        if (TMA) {
+            __syncthreads();                // (first tile: mbarriers initialised) previous tile's exchange reads are done
+            z_mbar_wait(&bars[0], sphase);  // this tile's input has landed
+            sphase ^= 1;
+        } else {
+            cp_async_wait<1>();             // this tile's input has landed (the newest group may still be in flight)
+            __syncthreads();                // ... for every thread; also: previous tile's exchange reads are done
+        }
         // ---- forward step 1: tasks (c, n2): R1-point over n1 (inputs in bit-reversed register order, k1 natural)
 #pragma unroll
         for (int it = 0; it < NT1; ++it) {
@@ -227,9 +301,10 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
         __syncthreads();                    // exchange written, staging buffer free
         if (nxt.valid(a)) {
             cur_base = tile_base(nxt);
-            prefetch_tile(cur_base);
+            if (TMA) { if (threadIdx.x == 0) tma_tile(nxt); }
+            else prefetch_tile(cur_base);
         }
-        cp_async_commit();                  // group A (possibly empty): input of the next tile
+        if (!TMA) cp_async_commit();        // group A (possibly empty): input of the next tile
         // ---- forward step 3 for thread k1 = tp: twiddle, R2-point over n2; u[c][p] = P~_c[k1 + R1 brev(p)]
         const int k1 = tp;
         cx<T> wk[R2];                       // w_M^{n2 k1}, n2 = 1 .. R2-1 (wk[0] unused)
@@ -248,7 +323,15 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
             });
             Dif<T, -1, R2>::run(u[c]);
         }
-        cp_async_wait<1>();                 // K~ of this item has landed (only the group just committed may be pending)
+        if (TMA) {
+            if (kpend) {                    // K~ of this item has landed
+                z_mbar_wait(&bars[1], kphase);
+                kphase ^= 1;
+                kpend = false;
+            }
+        } else {
+            cp_async_wait<1>();             // K~ of this item has landed (only the group just committed may be pending)
+        }
         __syncthreads();                    // ... for every thread; exchange fully read
         // ---- multiply
         {
@@ -291,7 +374,12 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
             }
         }
         __syncthreads();                    // exchange written; every thread is past the multiply: K~ buffer free
-        if (nxt.valid(a) && !nxt.same_item(cur)) {
+        if (TMA) {
+            if (nxt.valid(a) && !nxt.same_item(cur)) {
+                if (threadIdx.x == 0) tma_k(nxt);
+                kpend = true;
+            }
+        } else if (nxt.valid(a) && !nxt.same_item(cur)) {
             if constexpr (NIDLE > 0) {
                 if (tp >= 3 * R2)
                     prefetch_k(nxt, std::integral_constant<int, NIDLE>{}, std::integral_constant<int, 3 * R2 * LANES>{});
@@ -299,7 +387,7 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
                 prefetch_k(nxt, ic_all{}, ic_zero{});
             }
         }
-        cp_async_commit();                  // group B (possibly empty): K~ of the next item
+        if (!TMA) cp_async_commit();        // group B (possibly empty): K~ of the next item
         // ---- inverse step 2: tasks (c, n2): R1-point over k1, rows n1 R2 + n2 (n1 < R1/2 when pruned) stored
 #pragma unroll
         for (int it = 0; it < NT1; ++it) {
@@ -324,6 +412,46 @@ k2_zmul(cx<T>* __restrict__ S, const T* __restrict__ Kt, Z2Args a)
     cp_async_wait<0>();
 }
 
+// Tensor maps of the tiled spectra S[b][c][g][z][ky][L] (as reals: 2 L per row) and of the tiled table Kt[6][g][ky][kz][L]
+// with the boxes of one tile / one K~ tile.  False when the strides are not the tiled ones or the encoder is missing.
+template <typename T>
+static bool make_z_maps(void* S, const T* Kt, const Z2Args& a, int lanes, int nin, int hz, CUtensorMap* smap, CUtensorMap* kmap)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn enc = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            enc = reinterpret_cast<encode_fn>(fn);
+        tried = true;
+    }
+    if (!enc) return false;
+    const int64_t L = lanes, My = a.My, nz = a.nz, G = a.ngroups, Hy = a.My / 2 + 1;
+    if (a.s_ky != L || a.s_z != My * L || a.s_g != nz * My * L || a.cs != G * nz * My * L) return false;
+    if (a.k_skz != L || a.k_sky != hz * L || a.k_sg != Hy * hz * L || a.kcs != G * Hy * hz * L) return false;
+    if (hz > 256 || nin > 256) return false;
+    const CUtensorMapDataType dt = sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const cuuint32_t es[5] = {1, 1, 1, 1, 1};
+    const cuuint64_t row = (cuuint64_t)(2 * L * sizeof(T));                               // 128 bytes
+    const cuuint64_t sd[5] = {(cuuint64_t)(2 * L), (cuuint64_t)My, (cuuint64_t)nz, (cuuint64_t)G, (cuuint64_t)3 * a.batch};
+    const cuuint64_t ss[4] = {row, row * My, row * My * nz, row * My * nz * G};
+    const cuuint32_t sb[5] = {(cuuint32_t)(2 * L), 1, (cuuint32_t)nin, 1, 3};
+    if (enc(smap, dt, 5, S, sd, ss, sb, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    const cuuint64_t krow = (cuuint64_t)(L * sizeof(T));
+    const cuuint64_t kd[5] = {(cuuint64_t)L, (cuuint64_t)hz, (cuuint64_t)Hy, (cuuint64_t)G, 6};
+    const cuuint64_t ks[4] = {krow, krow * hz, krow * hz * Hy, krow * hz * Hy * G};
+    const cuuint32_t kb[5] = {(cuuint32_t)L, (cuuint32_t)hz, 1, 1, 6};
+    return enc(kmap, dt, 5, const_cast<T*>(Kt), kd, ks, kb, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <typename T, int M, int LANES, bool PRUNE>
 static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
 {
@@ -331,20 +459,28 @@ static cudaError_t launch_one(void* S, const T* Kt, Z2Args a, cudaStream_t st)
     static PerDevice<int> cache;
     int& nblocks = cache.here();
     if (!nblocks) {
-        cudaError_t e = cudaFuncSetAttribute(k2_zmul<T, M, LANES, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(k2_zmul<T, M, LANES, PRUNE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)C::smem);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(k2_zmul<T, M, LANES, PRUNE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem);
         if (e != cudaSuccess) return e;
         int dev = 0, sms = 0, per = 0;
         if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
         if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k2_zmul<T, M, LANES, PRUNE>, C::THREADS, C::smem)) !=
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k2_zmul<T, M, LANES, PRUNE, false>, C::THREADS, C::smem)) !=
             cudaSuccess)
             return e;
         nblocks = sms * (per > 0 ? per : 1);
     }
     a.nitems = a.ngroups * (a.My / 2 + 1);
     const int grid = a.nitems < nblocks ? a.nitems : nblocks;
-    k2_zmul<T, M, LANES, PRUNE><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a);
+    CUtensorMap smap, kmap;
+    memset(&smap, 0, sizeof(smap));
+    memset(&kmap, 0, sizeof(kmap));
+    if (make_z_maps<T>(S, Kt, a, LANES, C::NIN, C::HZ, &smap, &kmap))
+        k2_zmul<T, M, LANES, PRUNE, true><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a, smap, kmap);
+    else
+        k2_zmul<T, M, LANES, PRUNE, false><<<grid, C::THREADS, C::smem, st>>>(static_cast<cx<T>*>(S), Kt, a, smap, kmap);
     return cudaGetLastError();
 }
 
