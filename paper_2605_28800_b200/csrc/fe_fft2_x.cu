@@ -6,6 +6,8 @@
 // (the inverse is unnormalised; 1/(M m_y m_z) is folded into the tensor spectrum at precompute).
 // Each row is handled by R2 threads with the register two-level transform of fe_fft2.cuh.
 #include "fe_fft2.cuh"
+#include <string.h>
+#include <cuda.h>          // CUtensorMap and cuTensorMapEncodeTiled's signature only; the entry point is fetched at run time
 
 namespace fe {
 namespace v2 {
@@ -196,6 +198,188 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// k6_xinv: persistent inverse x pass for the tiled spectrum layout (fp64, Mc = 256).  The half spectra of a group of
+// ROWS rows ([g][row][L] in memory: one 3-D box) arrive by ONE tensor copy into a single shared-memory buffer; the rows
+// are transformed IN PLACE in that buffer: a row's R2 threads sit in one warp and own the row's 128-byte pieces, so the
+// exchange of the two-level transform needs only __syncwarp, and an XOR swizzle (column ^ (row of the exchange & 7))
+// replaces the padding column, which lets the 16 x 16 exchange fit into the 33 x 8 slots of the row.  As soon as every
+// thread holds its second-step inputs the buffer is free and thread 0 starts the copy of the block's next group, which
+// lands behind the second register FFT and the stores.
+// ------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned x6_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <typename T, int M, bool PRUNE>
+__global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a, int G, int nplanes,
+                                                  const __grid_constant__ CUtensorMap imap)
+{
+    using C = XCfg<M>;
+    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS, TWG = 8;
+    constexpr int L = 128 / (int)sizeof(cx<T>);
+    static_assert(R1 == TPP && L == 8, "one second-step task per thread, 8 complex per 128-byte piece");
+    cx<T>* buf = reinterpret_cast<cx<T>*>(fe2_smem);                       // [G][ROWS][L]
+    cx<T>* tw = buf + (size_t)G * ROWS * L;                               // w_M^(n2 k1) at [k1 * R2 + n2]
+    cx<T>* tws = tw + M;                                                  // w_2M^k
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tws + M);
+    const int t = threadIdx.x, tp = t % TPP, rl = t / TPP;
+    const int gpp = a.ny / ROWS;                                          // row groups per plane
+    const int ngroups = nplanes * gpp;
+    const unsigned bytes = (unsigned)((size_t)G * ROWS * L * sizeof(cx<T>));
+    auto issue = [&](int grp) {
+        const int plane = grp / gpp, y0 = (grp - plane * gpp) * ROWS;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(x6_smem_u32(bar)), "r"(bytes) : "memory");
+        asm volatile(
+            "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];\n" ::"r"(
+                x6_smem_u32(buf)),
+            "l"(&imap), "r"(0), "r"(y0), "r"(0), "r"(plane), "r"(x6_smem_u32(bar))
+            : "memory");
+    };
+    if (t == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(x6_smem_u32(bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        if ((int)blockIdx.x < ngroups) issue(blockIdx.x);
+    }
+    {
+        const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
+        for (int e = t; e < M; e += 256) {
+            tw[e] = twg[((e / R2) * (e % R2)) * (kTwiddleN / M)];
+            tws[e] = twg[e * (kTwiddleN / (2 * M))];
+        }
+    }
+    __syncthreads();
+    // element k of this thread's row / slot s of the row's in-place exchange
+    auto at = [&](int k) { return buf + ((k >> 3) * ROWS + rl) * L + (k & 7); };
+    unsigned phase = 0;
+    for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        {
+            const unsigned addr = x6_smem_u32(bar);
+            unsigned done;
+            do {
+                asm volatile(
+                    "{\n"
+                    ".reg .pred p;\n"
+                    "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+                    "selp.u32 %0, 1, 0, p;\n"
+                    "}\n"
+                    : "=r"(done)
+                    : "r"(addr), "r"(phase)
+                    : "memory");
+            } while (!done);
+            phase ^= 1;
+        }
+        cx<T> v[R1];
+        static_for<R1>([&](auto jc) {
+            constexpr int j1 = decltype(jc)::value;
+            const int k = tp + R2 * j1;
+            const cx<T> Xk = *at(k), Xn = *at(M - k);
+            const T ex = (T)0.5 * (Xk.x + Xn.x), ey = (T)0.5 * (Xk.y - Xn.y);
+            const T dx = (T)0.5 * (Xk.x - Xn.x), dy = (T)0.5 * (Xk.y + Xn.y);
+            const cx<T> w = tws[k];
+            const T ox = dx * w.x + dy * w.y, oy = dy * w.x - dx * w.y;   // D * conj(w)
+            v[j1] = {ex - oy, ey + ox};
+        });
+        Dif<T, +1, R1>::run(v);
+        __syncwarp();                       // every thread of the row has read its inputs: the row's slots are free
+        static_for<R1 / TWG>([&](auto gc) {
+            constexpr int g = decltype(gc)::value;
+            cx<T> w[TWG];
+            static_for<TWG>([&](auto qc) {
+                constexpr int o1 = brev<R1>(g * TWG + decltype(qc)::value);
+                if constexpr (o1 != 0) w[decltype(qc)::value] = tw[o1 * R2 + tp];
+            });
+            static_for<TWG>([&](auto qc) {
+                constexpr int p = g * TWG + decltype(qc)::value;
+                constexpr int o1 = brev<R1>(p);
+                cx<T> val = v[p];
+                if constexpr (o1 != 0) val = cmulc(val, w[decltype(qc)::value]);
+                *at(o1 * R2 + (tp ^ (o1 & 7))) = val;
+            });
+        });
+        __syncwarp();
+        const int o1 = tp;
+        cx<T> u[R2];
+        static_for<R2>([&](auto nc) { u[decltype(nc)::value] = *at(o1 * R2 + (decltype(nc)::value ^ (o1 & 7))); });
+        __syncthreads();                    // every row of the group is in registers: the buffer is free
+        if (t == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
+        Dif<T, +1, R2>::run(u);
+        const int plane = grp / gpp, y0 = (grp - plane * gpp) * ROWS;
+        const int64_t row = (int64_t)plane * a.ny + y0 + rl;
+        cx<T>* dst = reinterpret_cast<cx<T>*>(out + row * a.real_rs) + o1;
+        static_for<R2>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int o2 = brev<R2>(p);
+            if constexpr (!PRUNE || o2 < R2 / 2) {
+                if (!PRUNE || o1 + R1 * o2 < a.nc) dst[R1 * o2] = u[p];
+            }
+        });
+    }
+}
+
+// tensor map of the tiled half spectra S1[plane][g][y][L] (as reals) with the box of one row group; false if unavailable
+template <typename T>
+static bool make_x_map(const void* S1, int ny, int G, int nplanes, int rows, CUtensorMap* map)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn enc = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            enc = reinterpret_cast<encode_fn>(fn);
+        tried = true;
+    }
+    if (!enc || G > 256 || rows > 256) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)(128 / sizeof(T)), (cuuint64_t)ny, (cuuint64_t)G, (cuuint64_t)nplanes};
+    const cuuint64_t strides[3] = {128, (cuuint64_t)ny * 128, (cuuint64_t)G * ny * 128};
+    const cuuint32_t box[4] = {(cuuint32_t)(128 / sizeof(T)), (cuuint32_t)rows, (cuuint32_t)G, 1};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    return enc(map, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
+               const_cast<void*>(S1), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+// persistent tensor-copy inverse pass when the layout is the tiled one (fp64, Mc = 256, whole row groups per plane)
+template <typename T, bool PRUNE>
+static bool try_launch_xinv6(const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
+{
+    if constexpr (sizeof(T) != 8) {
+        return false;
+    } else {
+        constexpr int M = 256;
+        using C = XCfg<M>;
+        constexpr int L = 8;
+        if (a.lg != 3 || a.s_row != L || a.s_g != (int64_t)a.ny * L || a.ny % C::ROWS || a.s_plane % ((int64_t)a.ny * L)) return false;
+        const int G = (int)(a.s_plane / ((int64_t)a.ny * L));
+        if (a.nrows % a.ny) return false;
+        const int nplanes = (int)(a.nrows / a.ny);
+        CUtensorMap map;
+        memset(&map, 0, sizeof(map));
+        if (!make_x_map<T>(in, a.ny, G, nplanes, C::ROWS, &map)) return false;
+        const size_t smem = (size_t)G * C::ROWS * L * sizeof(cx<T>) + (size_t)2 * M * sizeof(cx<T>) + 16;
+        if (smem > 113 * 1024) return false;
+        static PerDevice<int> cache;
+        int& nblocks = cache.here();
+        if (!nblocks) {
+            cudaError_t e = cudaFuncSetAttribute(k6_xinv<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
+            int dev = 0, sms = 0, per = 0;
+            if (e == cudaSuccess) e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xinv<T, M, PRUNE>, 256, smem);
+            if (e != cudaSuccess) { *err = e; return true; }
+            nblocks = sms * (per > 0 ? per : 1);
+        }
+        const int ngroups = nplanes * (a.ny / C::ROWS);
+        const int grid = ngroups < nblocks ? ngroups : nblocks;
+        k6_xinv<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<T*>(out), a, G, nplanes, map);
+        *err = cudaGetLastError();
+        return true;
+    }
+}
+
 template <typename T, int M, bool PRUNE, bool FWD>
 static cudaError_t launch_one(const void* in, void* out, const X2Args& a, cudaStream_t st)
 {
@@ -271,6 +455,10 @@ cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, in
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
     v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2};
+    if (M == 256 && prune) {
+        cudaError_t e = cudaSuccess;
+        if (v2::try_launch_xinv6<T, true>(in, out, a, &e, st)) return e;
+    }
     return v2::launch_x<T, false>(M, prune, in, out, a, st);
 }
 
