@@ -234,6 +234,7 @@ def run_cuda(args):
     g.set_option(fe.FE_OPT_FUSE_XY, args.fuse_xy)
     if args.xy_ring:
         g.set_option(fe.FE_OPT_XY_RING, args.xy_ring)
+    g.set_option(fe.FE_OPT_XL_SLABS, args.xl_slabs)
     t0 = time.time()
     g.precompute_tensor()
     t_pre = time.time() - t0
@@ -300,7 +301,7 @@ def run_cuda(args):
     cdom = ctr.get(dom) if isinstance(ctr.get(dom), dict) else {}
     traffic = cdom.get("dram_bytes") if cdom else (ctr.get(dom) if not isinstance(ctr.get(dom), dict) else None)
     # kernel that serves the profile slot on the size-specialised path (every bench workload but cfg1 takes it)
-    fast_names = {"xfwd": "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>", "xinv": "k2_xinv",
+    fast_names = {"xfwd": "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>", "xinv": "k6_xinv",
                   "local": "k_local2", "xyfwd": "k_xyfwd", "xyinv": "k_xyinv"}
     generic = args.workload == "cfg1"
     # which roofline binds the dominant kernel: the largest of its fractions of the three measured unit peaks
@@ -403,7 +404,7 @@ def run_cuda(args):
                 "config": {"workload": w.name, "grid": list(w.n), "batch": w.batch, "integrator": "euler",
                            "terms": "landau+gradient+elec+ext", "padded_fft": padded_dims(w),
                            "l2": "state and spectra exceed L2 (P 3N reals, spectra >= 4x that)",
-                           "parallelism": "replicas x%d" % world, "fuse_xy": args.fuse_xy},
+                           "parallelism": "replicas x%d" % world, "fuse_xy": args.fuse_xy, "xl_slabs": args.xl_slabs},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                 "clocks": cs.summary(), "cufft_baseline": cufft, "precompute_s": t_pre,
                 "energy_after": {"F_tot": float(en[4]), "finite": bool(np.isfinite(en).all())}}
@@ -562,6 +563,8 @@ def main():
     ap.add_argument("--fuse-xy", type=int, default=0, choices=[0, 1],
                     help="FE_OPT_FUSE_XY: 1 = x and y passes fused through the L2 ring, 0 = separate kernels (default)")
     ap.add_argument("--xy-ring", type=int, default=0, help="FE_OPT_XY_RING (0 = automatic)")
+    ap.add_argument("--xl-slabs", type=int, default=0,
+                    help="FE_OPT_XL_SLABS: n > 1 = x inverse pass and local step slab by slab, E_elec handed over in L2")
     args = ap.parse_args()
     args.warmup_requested = args.warmup
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup

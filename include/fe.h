@@ -114,8 +114,13 @@ fe_status fe_set_material_map(fe_grid* g, const uint8_t* dev_map);
  *   FE_OPT_XY_TIMEOUTS read-only (fe_get_option synchronises the device): 1 if a wait inside the fused kernel ever
  *                      timed out (it cannot unless the device is shared with a kernel that never yields).
  *   FE_OPT_XY_RING     planes in the L2 ring of the fused pass; 0 (default) sizes it from the geometry (>= 24 planes,
- *                      <= 32 MB), 2..4096 fixes it (clamped to the number of planes). */
-enum { FE_OPT_FUSE_XY = 0, FE_OPT_XY_TIMEOUTS = 1, FE_OPT_XY_RING = 2 };
+ *                      <= 32 MB), 2..4096 fixes it (clamped to the number of planes).
+ *   FE_OPT_XL_SLABS    n > 1: inside fe_step / fe_rhs the inverse x transform and the local step run slab by slab over n
+ *                      slabs of z planes, E_elec of a slab handed over through the first planes of the workspace's E
+ *                      buffer, which every slab overwrites and which therefore stay in L2 ("consumed
+ *                      without a round trip") -- where the geometry allows it (fp64, padded x length 512, open x,
+ *                      ny a multiple of 16); 0 / 1 (default): one x-inverse launch writes E_elec for the whole grid. */
+enum { FE_OPT_FUSE_XY = 0, FE_OPT_XY_TIMEOUTS = 1, FE_OPT_XY_RING = 2, FE_OPT_XL_SLABS = 3 };
 fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value);
 fe_status fe_get_option(fe_grid* g, int32_t option, int32_t* value);
 

@@ -26,7 +26,7 @@ SYMBOLS = ["fe_create_grid", "fe_destroy_grid", "fe_workspace_bytes", "fe_bind_w
            "fe_version", "fe_profile", "fe_profile_read", "fe_step_rk45", "fe_set_external_wave", "fe_set_time",
            "fe_get_time", "fe_set_option", "fe_get_option"]
 KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other", "xyfwd", "xyinv"]
-FE_OPT_FUSE_XY, FE_OPT_XY_TIMEOUTS, FE_OPT_XY_RING = 0, 1, 2
+FE_OPT_FUSE_XY, FE_OPT_XY_TIMEOUTS, FE_OPT_XY_RING, FE_OPT_XL_SLABS = 0, 1, 2, 3
 
 
 class fe_rk45_stats(ctypes.Structure):

@@ -60,6 +60,7 @@ struct fe_grid {
     size_t ws_bytes;
     size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_K[6], o_part, o_cnt, o_box, o_Sbox, total_bytes;
     int opt_fuse_xy;                 // FE_OPT_FUSE_XY
+    int opt_xl_slabs;                // FE_OPT_XL_SLABS
     int opt_xy_ring;                 // FE_OPT_XY_RING (0: automatic)
     int nblk;
     bool tensor_ready;
@@ -244,6 +245,7 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     g->dirty = true;
     g->mixed = 0;
     g->opt_fuse_xy = 0;
+    g->opt_xl_slabs = 0;
     g->opt_xy_ring = 0;
     g->map = nullptr;
     g->ws = nullptr;
@@ -468,6 +470,11 @@ extern "C" fe_status fe_set_option(fe_grid* g, int32_t option, int32_t value)
         g->gvalid = false;
         return FE_OK;
     }
+    if (option == FE_OPT_XL_SLABS && value >= 0 && value <= 64) {
+        g->opt_xl_slabs = value;
+        g->gvalid = false;
+        return FE_OK;
+    }
     return fail(FE_EINVAL, "unknown option %d or bad value %d", option, value);
 }
 
@@ -476,6 +483,7 @@ extern "C" fe_status fe_get_option(fe_grid* g, int32_t option, int32_t* value)
     if (!g || !value) return fail(FE_EINVAL, "null argument");
     if (option == FE_OPT_FUSE_XY) { *value = g->opt_fuse_xy; return FE_OK; }
     if (option == FE_OPT_XY_RING) { *value = g->opt_xy_ring; return FE_OK; }
+    if (option == FE_OPT_XL_SLABS) { *value = g->opt_xl_slabs; return FE_OK; }
     if (option == FE_OPT_XY_TIMEOUTS) {
         *value = 0;
         if (!g->ws) return FE_OK;
@@ -577,7 +585,7 @@ extern "C" fe_status fe_get_tensor(fe_grid* g, double* host_out, void* stream)
 
 // ---- a1-a3: electrostatic field of state Y into the E buffer ------------------------------------------
 template <typename T>
-static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
+static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st, bool skip_xinv = false)
 {
     const Geometry& q = g->geo;
     const int B = g->desc.batch;
@@ -656,10 +664,12 @@ static fe_status elec_field(fe_grid* g, const T* Y, cudaStream_t st)
         FE_CUDA(launch_axis<T>(g->ctx, 1, +1, S2, S1, q.n[1], q.lanes, q.pitch, q.n[2], B * 3, p, p * q.m[1],
                                p * q.m[1] * q.n[2], p, p * q.n[1], p * q.n[1] * q.n[2], st));
     }
+    g->launches += 2;
+    if (skip_xinv) return FE_OK;         // the caller runs the x inverse pass slab by slab (FE_OPT_XL_SLABS)
     mark(g, K_XINV, st);
     if (g->fast[0]) FE_CUDA(launch_xinv2<T>(g->ctx, S1, E, nx, rows, nx, xspec, L, st));
     else FE_CUDA(launch_xinv<T>(g->ctx, S1, E, q.n[0], q.n[1], slabs, p, p * q.n[1], q.n[0], (int64_t)q.n[0] * q.n[1], st));
-    g->launches += 3;
+    g->launches += 1;
     return FE_OK;
 }
 
@@ -677,8 +687,16 @@ static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double c
                        uint32_t terms, cudaStream_t st, const StageLin* lin = nullptr)
 {
     const bool elec = (terms & FE_TERM_ELEC) != 0;
+    // FE_OPT_XL_SLABS > 1: E_elec goes from the x inverse pass to the local step slab by slab through the first
+    // planes of each component's region of the E buffer, which every slab overwrites and which so stay in L2 (no round trip through HBM)
+    const Geometry& q = g->geo;
+    const int Lx = (int)(128 / g->csz);
+    const int nslab = elec && g->opt_xl_slabs > 1 && g->fast[0] && g->tiled && q.n[2] >= g->opt_xl_slabs &&
+                              xinv_slab_supported(q.m[0] / 2, q.n[0], q.n[1], Lx, sizeof(T))
+                          ? g->opt_xl_slabs
+                          : 1;
     if (elec) {
-        fe_status s = elec_field<T>(g, Y, st);
+        fe_status s = elec_field<T>(g, Y, st, nslab > 1);
         if (s != FE_OK) return s;
     }
     LocalArgs a;
@@ -705,6 +723,24 @@ static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double c
     a.batch = g->desc.batch;
     a.mixed = g->mixed;
     a.t = g->tstage;
+    if (nslab > 1) {
+        const int64_t p = q.pitch;
+        const int nx = q.n[0], ny = q.n[1], nz = q.n[2];
+        const int64_t xspec[4] = {ny, p * ny, Lx, (int64_t)ny * Lx};      // tiled S1 as the x passes see it
+        for (int k = 0; k < nslab; ++k) {
+            const int zb = (int)((int64_t)nz * k / nslab), ze = (int)((int64_t)nz * (k + 1) / nslab);
+            mark(g, K_XINV, st);
+            FE_CUDA(launch_xinv2_slab<T>(g->ctx, g->ws + g->o_S1, reinterpret_cast<T*>(g->ws + g->o_E), nx, g->desc.batch * 3, ny,
+                                         nz, zb, ze - zb, xspec, Lx, st));
+            a.zbeg = zb;
+            a.zend = ze;
+            a.e_z0 = zb;
+            mark(g, K_LOCAL, st);
+            FE_CUDA(launch_local<T>(a, st));
+            g->launches += 2;
+        }
+        return FE_OK;
+    }
     mark(g, K_LOCAL, st);
     FE_CUDA(launch_local<T>(a, st));
     g->launches += 1;

@@ -22,6 +22,10 @@ struct X2Args {
     int ny, lg;
     int64_t s_plane, s_row, s_g;
     int nc;         // valid complex pairs (x[2j], x[2j+1]) per real row: n_x / 2 (<= M/2 on a zero-padded axis, M otherwise)
+    // k6_xinv on a slab of z planes: plane q of the launch reads spectrum plane (q / pl_n) * pl_full + pl_off + q % pl_n
+    // (pl_n planes of each of the B * 3 components, starting at z = pl_off of pl_full) and writes real plane
+    // (q / pl_n) * pl_full + q % pl_n (the first pl_n planes of the component's region); pl_n == 0: q itself for both
+    int pl_n, pl_full, pl_off;
 };
 __device__ __forceinline__ int64_t spec_off(const X2Args& a, int k) { return (int64_t)(k >> a.lg) * a.s_g + (k & ((1 << a.lg) - 1)); }
 __device__ __forceinline__ int64_t spec_row(const X2Args& a, int64_t row) { return (row / a.ny) * a.s_plane + (row % a.ny) * a.s_row; }
@@ -226,7 +230,9 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     const int ngroups = nplanes * gpp;
     const unsigned bytes = (unsigned)((size_t)G * ROWS * L * sizeof(cx<T>));
     auto issue = [&](int grp) {
-        const int plane = grp / gpp, y0 = (grp - plane * gpp) * ROWS;
+        int plane = grp / gpp;
+        const int y0 = (grp - plane * gpp) * ROWS;
+        if (a.pl_n) plane = (plane / a.pl_n) * a.pl_full + a.pl_off + plane % a.pl_n;
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(x6_smem_u32(bar)), "r"(bytes) : "memory");
         asm volatile(
             "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];\n" ::"r"(
@@ -302,7 +308,9 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
         __syncthreads();                    // every row of the group is in registers: the buffer is free
         if (t == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
         Dif<T, +1, R2>::run(u);
-        const int plane = grp / gpp, y0 = (grp - plane * gpp) * ROWS;
+        int plane = grp / gpp;
+        const int y0 = (grp - plane * gpp) * ROWS;
+        if (a.pl_n) plane = (plane / a.pl_n) * a.pl_full + plane % a.pl_n;
         const int64_t row = (int64_t)plane * a.ny + y0 + rl;
         cx<T>* dst = reinterpret_cast<cx<T>*>(out + row * a.real_rs) + o1;
         static_for<R2>([&](auto pc) {
@@ -356,9 +364,10 @@ static bool try_launch_xinv6(const void* in, void* out, const X2Args& a, cudaErr
         const int G = (int)(a.s_plane / ((int64_t)a.ny * L));
         if (a.nrows % a.ny) return false;
         const int nplanes = (int)(a.nrows / a.ny);
+        const int map_planes = a.pl_n ? nplanes / a.pl_n * a.pl_full : nplanes;
         CUtensorMap map;
         memset(&map, 0, sizeof(map));
-        if (!make_x_map<T>(in, a.ny, G, nplanes, C::ROWS, &map)) return false;
+        if (!make_x_map<T>(in, a.ny, G, map_planes, C::ROWS, &map)) return false;
         const size_t smem = (size_t)G * C::ROWS * L * sizeof(cx<T>) + (size_t)2 * M * sizeof(cx<T>) + 16;
         if (smem > 113 * 1024) return false;
         static PerDevice<int> cache;
@@ -462,6 +471,25 @@ cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, in
     return v2::launch_x<T, false>(M, prune, in, out, a, st);
 }
 
+// planes [zb, zb + zn) of every one of the `comps` (= B * 3) components into planes [0, zn) of out[comps][nz][ny][n_real] -- the
+// slab hand-over of FE_OPT_XL_SLABS.  Only the persistent tensor-copy kernel has the plane mapping: cudaErrorNotSupported elsewhere.
+template <typename T>
+cudaError_t launch_xinv2_slab(const FftCtx& c, const void* in, T* out, int n_real, int comps, int ny, int nz, int zb, int zn,
+                              const int64_t spec[4], int lanes, cudaStream_t st)
+{
+    const int M = c.plan[0].M;
+    if (M != 256 || n_real > M || (n_real & 1)) return cudaErrorNotSupported;
+    int lg = 0;
+    while ((1 << lg) < lanes) ++lg;
+    v2::X2Args a{c.tw, (int64_t)comps * zn * ny, n_real, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2, zn, nz, zb};
+    cudaError_t e = cudaSuccess;
+    if (v2::try_launch_xinv6<T, true>(in, out, a, &e, st)) return e;
+    return cudaErrorNotSupported;
+}
+bool xinv_slab_supported(int Mc, int n_real, int ny, int lanes, size_t elem) { return elem == 8 && Mc == 256 && n_real <= Mc && ny % 16 == 0 && lanes == 8; }
+
+template cudaError_t launch_xinv2_slab<double>(const FftCtx&, const void*, double*, int, int, int, int, int, int, const int64_t*, int, cudaStream_t);
+template cudaError_t launch_xinv2_slab<float>(const FftCtx&, const void*, float*, int, int, int, int, int, int, const int64_t*, int, cudaStream_t);
 template cudaError_t launch_xfwd2<double>(const FftCtx&, const double*, void*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);
 template cudaError_t launch_xfwd2<float>(const FftCtx&, const float*, void*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);
 template cudaError_t launch_xinv2<double>(const FftCtx&, const void*, double*, int, int64_t, int64_t, const int64_t*, int, cudaStream_t);

@@ -118,6 +118,10 @@ template <typename T>
 cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, int64_t nrows, int64_t real_rs,
                          const int64_t spec[4], int lanes, cudaStream_t st);
 template <typename T>
+cudaError_t launch_xinv2_slab(const FftCtx& c, const void* in, T* out, int n_real, int comps, int ny, int nz, int zb, int zn,
+                              const int64_t spec[4], int lanes, cudaStream_t st);
+bool xinv_slab_supported(int Mc, int n_real, int ny, int lanes, size_t elem);
+template <typename T>
 cudaError_t launch_axis2(const FftCtx& c, int axis, int dir, const void* in, void* out, int n_keep, int n0, int n1,
                          int batch, int64_t in_sa, int64_t in_s0, int64_t in_s1, int64_t in_sb, int64_t out_sa,
                          int64_t out_s0, int64_t out_s1, int64_t out_sb, cudaStream_t st);
@@ -178,6 +182,10 @@ struct LocalArgs {
     double id2[3];        // 1 / D_a^2
     double i4[3];         // 1 / (4 D_x D_y), 1 / (4 D_x D_z), 1 / (4 D_y D_z)
     int zchunk;           // planes per block
+    // z slab of this launch (FE_OPT_XL_SLABS: the x inverse pass hands E_elec to the local step slab by slab through the
+    // first planes of every component's region of the E buffer, which stay in L2).  zend == 0: all planes
+    int zbeg, zend;
+    int e_z0;             // Eelec holds plane z of a component at plane z - e_z0 of its region (0: the whole field)
 };
 template <typename T> cudaError_t launch_local(const LocalArgs& a, cudaStream_t st);
 

@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
     const int ntx = (nx + kTX - 1) / kTX;
     const int x0 = (blockIdx.x % ntx) * kTX, y0 = (blockIdx.x / ntx) * kTY;
-    const int z0 = blockIdx.y * a.zchunk, z1 = min(z0 + a.zchunk, nz);
+    const int z0 = a.zbeg + blockIdx.y * a.zchunk, z1 = min(z0 + a.zchunk, a.zend);
     const int b = blockIdx.z;
     const int t = threadIdx.x, tx = t & 31, ty = t >> 5;
     const int64_t nxy = (int64_t)nx * ny, N = nxy * nz;
@@ -400,7 +400,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
     const int ntx = (nx + k2TX - 1) / k2TX;
     const int x0 = (blockIdx.x % ntx) * k2TX, y0 = (blockIdx.x / ntx) * kTY;
-    const int z0 = blockIdx.y * a.zchunk, z1 = min(z0 + a.zchunk, nz);
+    const int z0 = a.zbeg + blockIdx.y * a.zchunk, z1 = min(z0 + a.zchunk, a.zend);
     const int b = blockIdx.z;
     const int t = threadIdx.x, tx = t & 31, ty = t >> 5;
     const int64_t nxy = (int64_t)nx * ny, N = nxy * nz;
@@ -766,10 +766,14 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     const bool two = a.n[0] >= k2TX;      // two cells per thread on rows of at least 64 cells
     const int ntx = two ? (a.n[0] + k2TX - 1) / k2TX : (a.n[0] + kTX - 1) / kTX, nty = (a.n[1] + kTY - 1) / kTY;
     // z chunk: as long as possible (halo planes are re-read per chunk) while the grid still fills the machine
-    int zc = a.n[2];
-    while (zc > 8 && (int64_t)ntx * nty * ((a.n[2] + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
+    if (a.zend <= 0) { a.zbeg = 0; a.zend = a.n[2]; }
+    // a slab buffer holds plane z of a component at plane z - e_z0 of the component's region: fold that into the pointer
+    if (a.Eelec && a.e_z0) a.Eelec = static_cast<const T*>(a.Eelec) - (int64_t)a.e_z0 * a.n[0] * a.n[1];
+    const int nzl = a.zend - a.zbeg;      // planes of this launch
+    int zc = nzl;
+    while (zc > 8 && (int64_t)ntx * nty * ((nzl + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
     a.zchunk = zc;
-    dim3 grid(ntx * nty, (a.n[2] + zc - 1) / zc, a.batch);
+    dim3 grid(ntx * nty, (nzl + zc - 1) / zc, a.batch);
     const int ns = a.map ? 4 : 5;         // ring slots of k_local2
     const size_t smem = two ? (size_t)ns * k2_slot_bytes<T>() + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1) + 8 + ns * 8
                             : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);

@@ -297,3 +297,40 @@ def test_fused_xy_pass_through_the_l2_ring(fe, n, batch, dtype):
     assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < (1e-12 if dtype == "f64" else 1e-4)
     assert g.get_option(fe.FE_OPT_XY_TIMEOUTS) == 0
     g.close()
+
+
+@pytest.mark.parametrize("n,batch,slabs", [
+    ((256, 256, 32), 1, 4),           # the x kernels of config 5a, four slabs of 8 planes
+    ((256, 128, 24), 2, 5),           # two members, slabs of 4 / 5 planes
+    ((256, 64, 32), 1, 32),           # one plane per slab
+])
+def test_x_inverse_hands_e_elec_to_the_local_step_slab_by_slab(fe, n, batch, slabs):
+    """FE_OPT_XL_SLABS (E_elec "consumed without a round trip"): the x inverse pass and the local step
+    run slab by slab, E_elec of a slab in the first planes of the E buffer.  Against the oracle, against the unsliced path (bitwise: the
+    same kernels compute the same cells), every integrator's stage epilogue, and under graph replay."""
+    w = _workload(n, batch=batch)
+    o = orc.Oracle(oracle_problem(w, batch - 1), elec="fft")
+    want = o.rhs(w.P0[batch - 1], fi.TERM_ALL)
+    g = fe.Grid.from_workload(w, dtype="f64")
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    res = {}
+    for s in (slabs, 0):
+        g.set_option(fe.FE_OPT_XL_SLABS, s)
+        assert g.get_option(fe.FE_OPT_XL_SLABS) == s
+        g.profile(True)
+        res[s] = g.rhs(P, fi.TERM_ALL).cpu().numpy()
+        counts = {k: cnt for k, (ms, cnt) in g.profile_read().items()}
+        g.profile(False)
+        assert counts["xinv"] == counts["local"] == (s if s else 1)
+        assert rel_l2(res[s][batch - 1], want) < TOL_RHS64
+    assert np.array_equal(res[slabs], res[0])
+    for integ, nst in ((fi.EULER, 12), (fi.HEUN, 4), (fi.RK4, 3), (fi.AB3M2, 5)):
+        g.set_option(fe.FE_OPT_XL_SLABS, slabs)
+        Pa = g.state(w.P0)
+        g.step(Pa, w.dt, nst, integ, fi.TERM_ALL)
+        g.set_option(fe.FE_OPT_XL_SLABS, 0)
+        Pb = g.state(w.P0)
+        g.step(Pb, w.dt, nst, integ, fi.TERM_ALL)
+        assert np.array_equal(Pa.cpu().numpy(), Pb.cpu().numpy())
+    g.close()
