@@ -490,7 +490,23 @@ def oracle_steps(workload: str, steps: int, warmup: int, threads: int):
     for _ in range(steps):
         P = o.step(P, w.dt, 1, fi.EULER, fi.TERM_ALL)
     dt = time.perf_counter() - t0
+    oracle_steps.last = (o, P, w)
     return w, dt
+
+
+def oracle_single_thread_step():
+    """One more Euler step of the oracle object just timed, on ONE host thread (numpy.fft, one OpenMP thread): the
+    single-thread figure beside the all-cores one.  Returns seconds, or None when the OpenMP runtime cannot be reached."""
+    import ctypes
+    o, P, w = oracle_steps.last
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(1)
+    except OSError:
+        return None
+    o.fft_workers = None
+    t0 = time.perf_counter()
+    o.step(P, w.dt, 1, fi.EULER, fi.TERM_ALL)
+    return time.perf_counter() - t0
 
 
 def host_threads() -> int:
@@ -505,7 +521,9 @@ def cpu_baseline(workload: str):
     member of config 5b, 3 Euler steps after 1 warm-up step; tensor table outside the timed region."""
     th = host_threads()
     w, dt = oracle_steps(workload, 3, 1, th)
+    dt1 = oracle_single_thread_step()
     return {"value": w.cells * 3 / dt, "unit": UNIT, "cores": th, "kind": "oracle",
+            "single_thread_value": (w.cells / dt1) if dt1 else None,
             "sample": "%s: %dx%dx%d cells of the same recipe, 3 Euler steps, oracle-FFT electrostatics (scipy.fft, %d workers) "
                       "+ OpenMP C loops for Landau / gradient; tensor table built outside the timed region"
                       % (w.name, *w.n, th), "host_cores": os.cpu_count()}
