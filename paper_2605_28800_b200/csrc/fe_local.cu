@@ -380,9 +380,13 @@ template <typename T> __host__ __device__ constexpr size_t k2_slot_bytes() { ret
 // TMA = true (no material map, no periodic axis): a plane of the halo tile arrives as ONE tensor copy
 // (cp.async.bulk.tensor, box 68 x 10 x 1 x 3 components starting at (x0 - 2, y0 - 1, z); cells outside the sample are
 // zero-filled by the copy engine) issued by one thread and completed on an mbarrier, instead of four cp.async per thread.
-template <typename T, bool MAP, bool MIXED, bool TMA = false>
+// PLAIN = true: the forward-Euler stage with all four terms (terms == FE_TERM_ALL with E_elec, baseY == Y, no accumulator,
+// no folded stage combination, no raw-k output) -- the runtime switches of the epilogue become compile-time constants, which
+// frees the registers their pointers and flags hold and with them the per-plane recomputation of loop invariants.
+template <typename T, bool MAP, bool MIXED, bool TMA = false, bool PLAIN = false>
 __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_constant__ CUtensorMap tmap)
 {
+    static_assert(!(PLAIN && MAP), "the plain variant has no material map");
     extern __shared__ __align__(128) unsigned char lsm[];
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
     // three planes ahead of their use; with a map the loader goes through registers (vacuum cells are zeroed).
@@ -544,12 +548,14 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
         async_plane(z0 + 2);
     }
 
+    // the tensor-copy loader runs on open grids only: the boundary tests need no periodic flags there
+    const bool per0 = !TMA && a.periodic[0], per1 = !TMA && a.periodic[1], per2 = !TMA && a.periodic[2];
     const int x = x0 + 2 * tx, y = y0 + ty;          // cells (x, y) and (x + 1, y)
     const bool inside = x < nx && y < ny;            // nx is even: both cells or none
     const int64_t rxy = (int64_t)y * nx + x;
     const int c0 = (ty + 1) * k2PX + 2 + 2 * tx;
-    const T gxfA = (T)((x > 0 || a.periodic[0]) + 1), gxfB = (T)(1 + (x + 2 < nx || a.periodic[0]));
-    const T gyf = (T)((y > 0 || a.periodic[1]) + (y < ny - 1 || a.periodic[1]));
+    const T gxfA = (T)((x > 0 || per0) + 1), gxfB = (T)(1 + (x + 2 < nx || per0));
+    const T gyf = (T)((y > 0 || per1) + (y < ny - 1 || per1));
     const T G11 = (T)mem.G11, Gt = (T)mem.Gt, Gm = (T)mem.Gm, L = (T)mem.L;
     const T ix = (T)a.id2[0], iy = (T)a.id2[1], iz = (T)a.id2[2];
     const T qxy = Gm * (T)a.i4[0], qxz = Gm * (T)a.i4[1], qyz = Gm * (T)a.i4[2];
@@ -557,56 +563,72 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     const double wv = mem.wave ? sin(mem.womega * a.t + mem.wphase) : 0.0;      // E_ext sampled at the stage time
     const T ex0 = (T)(mem.Eext[0] + mem.wamp[0] * wv), ex1 = (T)(mem.Eext[1] + mem.wamp[1] * wv),
             ex2 = (T)(mem.Eext[2] + mem.wamp[2] * wv);
-    const T* Ee = (a.terms & 4u) && a.Eelec ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
-    const T* base = a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
-    const bool base_is_Y = a.baseY == a.Y;
+    const uint32_t terms = PLAIN ? 15u : a.terms;
+    const T* Ee = PLAIN || ((terms & 4u) && a.Eelec) ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
+    const T* base = PLAIN ? Y : a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
+    const bool base_is_Y = PLAIN || a.baseY == a.Y;
     T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
-    const T* ai = a.accOut ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
-    T* ao = a.accOut ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
+    const T* ai = !PLAIN && a.accOut ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
+    T* ao = !PLAIN && a.accOut ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
+    const int nlin = PLAIN ? 0 : a.nlin;
     const LandauD<T> lc0 = smats[0];
     auto ldp = [](const T* q) { return *reinterpret_cast<const P2*>(q); };
 
-    P2 en[3] = {{0, 0}, {0, 0}, {0, 0}};
-    if (Ee && inside) {
-        const int64_t r = (int64_t)z0 * nxy + rxy;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + r);
+    // PLAIN: the thread's own cell pair of planes z-1 and z rides in registers from plane to plane (6 of the 45 loads)
+    P2 cz[3] = {{0, 0}, {0, 0}, {0, 0}}, cc[3] = {{0, 0}, {0, 0}, {0, 0}};
+    if (PLAIN && !TMA) {
+        asm volatile("cp.async.wait_group 2;\n" ::);            // planes z0 - 1 and z0 of the four requested have landed
+        __syncthreads();
     }
-    for (int z = z0; z < z1; ++z) {
+    if (PLAIN && inside) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            cz[i] = ldp(tiles + i * k2Tile + c0);               // plane z0 - 1 sits in slot 0,
+            cc[i] = ldp(tiles + SLOT + i * k2Tile + c0);        // plane z0 in slot 1
+        }
+    }
+    // slots of planes z-1, z, z+1 and the phase bits of the slots' mbarriers, carried from plane to plane (no division per plane)
+    int sm1 = 0, s00 = 1, sp1 = 2;
+    unsigned phases = 3u;                            // slots 0 and 1 were awaited once in the prologue
+    int64_t r = (int64_t)z0 * nxy + rxy;             // cell pair (x, y, z) of this thread
+    for (int z = z0; z < z1; ++z, r += nxy, sm1 = s00, s00 = sp1, sp1 = (sp1 + 1 == NS ? 0 : sp1 + 1)) {
         if (MAP) {
             store_plane(z + 1);
             __syncthreads();
             if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
         } else if (TMA) {
-            tma_wait(z + 1);                                 // planes <= z+1 have landed
+            l_mbar_wait(&bars[sp1], (phases >> sp1) & 1u);   // planes <= z+1 have landed
+            phases ^= 1u << sp1;
             __syncthreads();                                 // every thread is done with plane z-2
-            tma_plane(z + 3);                                // into the slot of plane z-2
+            if (t == 0 && z + 3 <= z1) {                     // plane z+3 into the slot of plane z-2
+                const int s3 = sp1 + 2 >= NS ? sp1 + 2 - NS : sp1 + 2;
+                l_mbar_expect_tx(&bars[s3], (unsigned)(3 * k2Tile * sizeof(T)));
+                l_tma_load_4d(tiles + s3 * SLOT, &tmap, x0 - 2, y0 - 1, z + 3, 3 * b, &bars[s3]);
+            }
         } else {
             asm volatile("cp.async.wait_group 1;\n" ::);     // planes <= z+1 have landed
             __syncthreads();
             async_plane(z + 3);                              // into the slot of plane z-2 (commits a group)
         }
         if (!inside) continue;
-        const P2 ec[3] = {en[0], en[1], en[2]};
-        if (Ee && z + 1 < z1) {
-            const int64_t rn = (int64_t)(z + 1) * nxy + rxy;
+        // E_elec of this plane: requested here, consumed after the stencil
+        P2 ec[3] = {{0, 0}, {0, 0}, {0, 0}};
+        if (Ee) {
 #pragma unroll
-            for (int i = 0; i < 3; ++i) en[i] = ldp(Ee + i * N + rn);
+            for (int i = 0; i < 3; ++i) ec[i] = ldp(Ee + i * N + r);
         }
-        const int sm1 = slot_of(z - 1), s00 = slot_of(z), sp1 = slot_of(z + 1);
         const T* m0 = tiles + sm1 * SLOT;           // plane z-1
         const T* c = tiles + s00 * SLOT;            // plane z
         const T* p1 = tiles + sp1 * SLOT;           // plane z+1
         const unsigned char* fm = flags + sm1 * k2Tile;
         const unsigned char* fc = flags + s00 * k2Tile;
         const unsigned char* fp = flags + sp1 * k2Tile;
-        const int64_t r = (int64_t)z * nxy + rxy;
         const bool actA = !MAP || fc[c0], actB = !MAP || fc[c0 + 1];
         T EA[3] = {0, 0, 0}, EB[3] = {0, 0, 0};
         P2 pc[3];
 #pragma unroll
-        for (int i = 0; i < 3; ++i) pc[i] = ldp(c + i * k2Tile + c0);
-        if (a.terms & 1u) {
+        for (int i = 0; i < 3; ++i) pc[i] = PLAIN ? cc[i] : ldp(c + i * k2Tile + c0);
+        if (terms & 1u) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const LandauD<T> lc = MAP ? smats[a.map[r + h]] : lc0;
@@ -621,9 +643,9 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
                 E[2] -= pz * lc.dfd(lc.k1z, C, C2, A + B, A2 + B2, A * B, A3 + B3);
             }
         }
-        if (a.terms & 2u) {
+        if (terms & 2u) {
             // number of existing neighbours per axis (a missing neighbour holds 0 in the tile)
-            const T nzg = (T)((z > 0 || a.periodic[2]) + (z < nz - 1 || a.periodic[2]));
+            const T nzg = (T)((z > 0 || per2) + (z < nz - 1 || per2));
             const T nxA = MAP ? (T)(fc[c0 - 1] + fc[c0 + 1]) : gxfA, nxB = MAP ? (T)(fc[c0] + fc[c0 + 2]) : gxfB;
             const T nyA = MAP ? (T)(fc[c0 - k2PX] + fc[c0 + k2PX]) : gyf;
             const T nyB = MAP ? (T)(fc[c0 + 1 - k2PX] + fc[c0 + 1 + k2PX]) : gyf;
@@ -636,8 +658,9 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
                 const T* ci = c + i * k2Tile + c0;
                 dn[i] = ldp(ci - k2PX);
                 up[i] = ldp(ci + k2PX);
-                zm[i] = ldp(m0 + i * k2Tile + c0);
+                zm[i] = PLAIN ? cz[i] : ldp(m0 + i * k2Tile + c0);
                 zp[i] = ldp(p1 + i * k2Tile + c0);
+                if (PLAIN) { cz[i] = pc[i]; cc[i] = zp[i]; }
                 lf[i] = ci[-1];
                 rt[i] = ci[2];
                 const T gx_ = (i == 0 ? G11 : Gt) * ix, gy_ = (i == 1 ? G11 : Gt) * iy, gz_ = (i == 2 ? G11 : Gt) * iz;
@@ -684,7 +707,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
 #pragma unroll
             for (int i = 0; i < 3; ++i) { EA[i] += ec[i].a; EB[i] += ec[i].b; }
         }
-        if (a.terms & 8u) {
+        if (terms & 8u) {
             EA[0] += ex0; EA[1] += ex1; EA[2] += ex2;
             EB[0] += ex0; EB[1] += ex1; EB[2] += ex2;
         }
@@ -693,7 +716,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             if (actA) kA[i] = L * EA[i];
             if (actB) kB[i] = L * EB[i];
         }
-        if (a.kOut) {
+        if (!PLAIN && a.kOut) {
             T* ko = static_cast<T*>(a.kOut) + (int64_t)b * 3 * N;
 #pragma unroll
             for (int i = 0; i < 3; ++i) *reinterpret_cast<P2*>(ko + i * N + r) = P2{kA[i], kB[i]};
@@ -706,7 +729,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
                 if (base_is_Y && actA && actB) bv = pc[i];
                 else bv = ldp(base + i * N + r);
             }
-            for (int j = 0; j < a.nlin; ++j) {
+            for (int j = 0; j < nlin; ++j) {
                 const P2 lv = ldp(static_cast<const T*>(a.lk[j]) + (int64_t)b * 3 * N + i * N + r);
                 const T cj = (T)a.lc[j];
                 bv = P2{bv.a + cj * lv.a, bv.b + cj * lv.b};
@@ -796,6 +819,10 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e != cudaSuccess) return e;
         configured = 1;
     }
@@ -803,11 +830,19 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
         if (a.map) {
             if (a.mixed) k_local2<T, true, true><<<grid, 256, smem, st>>>(a, tmap);
             else k_local2<T, true, false><<<grid, 256, smem, st>>>(a, tmap);
-        } else if (tma) {
-            if (a.mixed) k_local2<T, false, true, true><<<grid, 256, smem, st>>>(a, tmap);
-            else k_local2<T, false, false, true><<<grid, 256, smem, st>>>(a, tmap);
         } else {
-            if (a.mixed) k_local2<T, false, true><<<grid, 256, smem, st>>>(a, tmap);
+            // forward-Euler stage with all four terms: the specialised epilogue (see k_local2)
+            const bool plain = a.terms == 15u && a.Eelec && a.baseY == a.Y && !a.accOut && !a.kOut && a.nlin == 0;
+            if (tma) {
+                if (plain) {
+                    if (a.mixed) k_local2<T, false, true, true, true><<<grid, 256, smem, st>>>(a, tmap);
+                    else k_local2<T, false, false, true, true><<<grid, 256, smem, st>>>(a, tmap);
+                } else if (a.mixed) k_local2<T, false, true, true><<<grid, 256, smem, st>>>(a, tmap);
+                else k_local2<T, false, false, true><<<grid, 256, smem, st>>>(a, tmap);
+            } else if (plain) {
+                if (a.mixed) k_local2<T, false, true, false, true><<<grid, 256, smem, st>>>(a, tmap);
+                else k_local2<T, false, false, false, true><<<grid, 256, smem, st>>>(a, tmap);
+            } else if (a.mixed) k_local2<T, false, true><<<grid, 256, smem, st>>>(a, tmap);
             else k_local2<T, false, false><<<grid, 256, smem, st>>>(a, tmap);
         }
         return cudaGetLastError();
