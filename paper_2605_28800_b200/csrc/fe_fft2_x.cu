@@ -255,6 +255,15 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     __syncthreads();
     // element k of this thread's row / slot s of the row's in-place exchange
     auto at = [&](int k) { return buf + ((k >> 3) * ROWS + rl) * L + (k & 7); };
+    // the swizzled exchange addresses depend on the thread only through eight bases each (no shift / xor per access)
+    static_assert(R2 == 2 * L, "two 128-byte pieces per exchange row");
+    cx<T>* wb[8];       // element (tp ^ c) of the row's first piece: the write of exchange row o1 lands o1 * 2 pieces further
+    cx<T>* rbp[8];      // element ((n & 7) ^ (tp & 7)) of exchange row tp: the read of column n adds its piece (n >> 3)
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        wb[c] = at(tp ^ c);
+        rbp[c] = at(tp * R2 + (c ^ (tp & 7)));
+    }
     unsigned phase = 0;
     for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
         {
@@ -298,13 +307,16 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
                 constexpr int o1 = brev<R1>(p);
                 cx<T> val = v[p];
                 if constexpr (o1 != 0) val = cmulc(val, w[decltype(qc)::value]);
-                *at(o1 * R2 + (tp ^ (o1 & 7))) = val;
+                wb[o1 & 7][o1 * (R2 / L) * ROWS * L] = val;      // = *at(o1 * R2 + (tp ^ (o1 & 7)))
             });
         });
         __syncwarp();
         const int o1 = tp;
         cx<T> u[R2];
-        static_for<R2>([&](auto nc) { u[decltype(nc)::value] = *at(o1 * R2 + (decltype(nc)::value ^ (o1 & 7))); });
+        static_for<R2>([&](auto nc) {                 // = *at(o1 * R2 + (n ^ (o1 & 7))), n = 8 (n >> 3) + (n & 7)
+            constexpr int n = decltype(nc)::value;
+            u[n] = rbp[n & 7][(n >> 3) * ROWS * L];
+        });
         __syncthreads();                    // every row of the group is in registers: the buffer is free
         if (t == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
         Dif<T, +1, R2>::run(u);
