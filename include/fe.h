@@ -159,6 +159,21 @@ fe_status fe_step_rk45(fe_grid* g, void* P, double t_span, double dt_init, doubl
  * over active cells.  Returns FE_ENONFINITE if any value is NaN/Inf (host_out is still written). */
 fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double* host_out, void* cuda_stream);
 
+/* fe_energy for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same kernels, same eight numbers per member, but
+ *   - dev_out is DEVICE memory, [B][8] doubles, caller-owned; nothing is copied to the host and the stream is NOT
+ *     synchronised (so no FE_ENONFINITE check either: the caller inspects the numbers);
+ *   - the per-block partial sums live in a file-scope static device array of the library (512 KiB, held by every GPU
+ *     that loads the library until the process exits) instead of the workspace; the call makes no cudaMalloc / cudaFree
+ *     and calls no allocating routine.
+ * Limit: batch * 296 * 8 partial sums must fit the 65536 doubles of that array, i.e. batch <= 27; beyond that the call
+ * returns FE_EINVAL with the numbers in fe_last_error.  All grids and all calls on a device SHARE the array: calls that
+ * may overlap on the GPU (different streams without an ordering between them) race on it; calls on one stream, or
+ * ordered by events, are safe.  The array keeps the last call's contents; every row a call reads is first written by
+ * that call, so nothing needs clearing.  With FE_TERM_ELEC the bound workspace is used as in fe_energy (E buffer and
+ * spectra; caller-owned memory).  PAPER.md:37 Eq. 2, 66 Eq. 5, 80 Eq. 7. */
+fe_status fe_energy_noalloc(fe_grid* g, const void* P, uint32_t terms, double* dev_out, void* cuda_stream);
+
 /* Test hooks. */
 /* host_out: [6][mz][my][mx] doubles (xx yy zz xy xz yz), the real-space kernel on the circular padded
  * box (m = 2n open, n periodic; entry at index (d mod m) holds K(d)). */

@@ -24,7 +24,7 @@ SYMBOLS = ["fe_create_grid", "fe_destroy_grid", "fe_workspace_bytes", "fe_bind_w
            "fe_set_global", "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs",
            "fe_step", "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_launch_count", "fe_last_error",
            "fe_version", "fe_profile", "fe_profile_read", "fe_step_rk45", "fe_set_external_wave", "fe_set_time",
-           "fe_get_time", "fe_set_option", "fe_get_option"]
+           "fe_get_time", "fe_set_option", "fe_get_option", "fe_energy_noalloc"]
 KERNEL_KINDS = ["xfwd", "yfwd", "zmul", "yinv", "xinv", "local", "other", "xyfwd", "xyinv"]
 FE_OPT_FUSE_XY, FE_OPT_XY_TIMEOUTS, FE_OPT_XY_RING, FE_OPT_XL_SLABS = 0, 1, 2, 3
 
@@ -88,6 +88,7 @@ def load():
         L.fe_rhs.argtypes = [vp, vp, vp, u32, vp]
         L.fe_step.argtypes = [vp, vp, dbl, i32, i32, u32, vp]
         L.fe_energy.argtypes = [vp, vp, u32, ctypes.POINTER(dbl), vp]
+        L.fe_energy_noalloc.argtypes = [vp, vp, u32, vp, vp]
         L.fe_get_tensor.argtypes = [vp, ctypes.POINTER(dbl), vp]
         L.fe_padded_dims.argtypes = [vp, ctypes.POINTER(i32)]
         L.fe_profile.argtypes = [vp, i32]
@@ -105,7 +106,7 @@ def load():
         for name in ("fe_create_grid", "fe_destroy_grid", "fe_bind_workspace", "fe_set_material", "fe_set_global",
                      "fe_set_external_field", "fe_set_material_map", "fe_precompute_tensor", "fe_rhs", "fe_step",
                      "fe_energy", "fe_get_tensor", "fe_padded_dims", "fe_profile", "fe_profile_read", "fe_set_option",
-                     "fe_get_option"):
+                     "fe_get_option", "fe_energy_noalloc"):
             getattr(L, name).restype = ctypes.c_int
         _lib = L
     return _lib
@@ -216,6 +217,14 @@ def fe_energy(h, P: torch.Tensor, batch: int, terms: int = FE_TERM_ALL, allow_no
     out = np.zeros((batch, 8), dtype=np.float64)
     _check(load().fe_energy(h, ctypes.c_void_p(P.data_ptr()), terms, out.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
                             _stream()), allow=(FE_ENONFINITE,) if allow_nonfinite else ())
+    return out
+
+
+def fe_energy_noalloc(h, P: torch.Tensor, out: torch.Tensor, terms: int = FE_TERM_ALL) -> torch.Tensor:
+    """fe_energy without allocation, host copy or synchronisation: `out` is a DEVICE float64 tensor [B][8] (include/fe.h)."""
+    if out.dtype != torch.float64 or not out.is_cuda or not out.is_contiguous() or out.device != P.device:
+        raise ValueError("out must be a contiguous float64 CUDA tensor on the state's device")
+    _check(load().fe_energy_noalloc(h, ctypes.c_void_p(P.data_ptr()), terms, ctypes.c_void_p(out.data_ptr()), _stream()))
     return out
 
 
@@ -341,6 +350,12 @@ class Grid:
     def energy(self, P: torch.Tensor, terms=FE_TERM_ALL, allow_nonfinite=False) -> np.ndarray:
         self._state_ok(P)
         return fe_energy(self.h, P, self.batch, terms, allow_nonfinite)
+
+    def energy_noalloc(self, P: torch.Tensor, out: torch.Tensor, terms=FE_TERM_ALL) -> torch.Tensor:
+        self._state_ok(P)
+        if tuple(out.shape) != (self.batch, 8):
+            raise ValueError("out must have shape (batch, 8)")
+        return fe_energy_noalloc(self.h, P, out, terms)
 
     def get_tensor(self) -> np.ndarray: return fe_get_tensor(self.h)
     def launch_count(self) -> int: return fe_launch_count(self.h)

@@ -1041,6 +1041,57 @@ extern "C" fe_status fe_energy(fe_grid* g, const void* P, uint32_t terms, double
     return FE_OK;
 }
 
+// ---- a6 without any allocation: partial sums in a static device array ---------------------------------
+// Scratch of fe_energy_noalloc: [B][nblk][8] partial sums of k_energy.  File-scope device memory: every GPU that loads the
+// library holds these 512 KiB until the process exits.  In host code the NAME of the array is a host-side stand-in, not a
+// device address; the address a kernel may use comes from cudaGetSymbolAddress, once per device with that device current.
+constexpr size_t kNoAllocDoubles = 65536;                               // 512 KiB: batch * 296 blocks * 8 sums, batch <= 27
+static __device__ __align__(256) double g_noalloc_partials[kNoAllocDoubles];
+
+extern "C" fe_status fe_energy_noalloc(fe_grid* g, const void* P, uint32_t terms, double* dev_out, void* stream)
+{
+    fe_status s = check_ready(g, P, terms);
+    if (s != FE_OK) return s;
+    if (!dev_out) return fail(FE_EINVAL, "null argument");
+    const size_t need = (size_t)g->desc.batch * g->nblk * 8;
+    if (need > kNoAllocDoubles)
+        return fail(FE_EINVAL, "fe_energy_noalloc: batch %d needs %zu partial sums, the static scratch holds %zu (batch <= %zu)",
+                    g->desc.batch, need, kNoAllocDoubles, kNoAllocDoubles / ((size_t)g->nblk * 8));
+    static PerDevice<double*> cache;                                    // device address of the array, per device
+    double*& scratch = cache.here();
+    if (!scratch) {
+        double* ptr = nullptr;
+        FE_CUDA(cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_noalloc_partials));
+        if (!ptr) return fail(FE_ECUDA, "cudaGetSymbolAddress returned a null address");
+        scratch = ptr;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((s = sync_params(g, st)) != FE_OK) return s;
+    const bool elec = (terms & FE_TERM_ELEC) != 0;
+    if (elec) {
+        s = g->f32 ? elec_field<float>(g, (const float*)P, st) : elec_field<double>(g, (const double*)P, st);
+        if (s != FE_OK) return s;
+    }
+    EnergyArgs a;
+    memset(&a, 0, sizeof(a));
+    a.P = P;
+    a.Eelec = elec ? g->ws + g->o_E : nullptr;
+    a.map = g->map;
+    a.mats = g->d_mats;
+    a.members = g->d_members;
+    a.nmat = g->desc.n_materials;
+    for (int i = 0; i < 3; ++i) { a.n[i] = g->geo.n[i]; a.periodic[i] = g->geo.periodic[i]; a.d[i] = g->geo.d[i]; }
+    a.terms = terms;
+    a.batch = g->desc.batch;
+    a.partials = scratch;             // every row [b][block][0..7] is written by its block before it is summed: nothing to clear
+    a.out = dev_out;
+    a.nblk = g->nblk;
+    a.t = g->time;
+    FE_CUDA(g->f32 ? launch_energy<float>(a, st) : launch_energy<double>(a, st));
+    g->launches += 2;
+    return FE_OK;
+}
+
 // ---- per-kernel timing (bench.py's roofline leg) ------------------------------------------------------
 extern "C" fe_status fe_profile(fe_grid* g, int32_t enable)
 {
