@@ -8,6 +8,7 @@
 //   then the integrator stage:  Yout = baseY + cy * k,  accOut = accIn + ca * k
 #include "fe_internal.h"
 #include <string.h>
+#include <type_traits>
 #include <cuda.h>          // CUtensorMap and cuTensorMapEncodeTiled's signature only; the entry point is fetched at run time
 
 namespace fe {
@@ -380,13 +381,18 @@ template <typename T> __host__ __device__ constexpr size_t k2_slot_bytes() { ret
 // TMA = true (no material map, no periodic axis): a plane of the halo tile arrives as ONE tensor copy
 // (cp.async.bulk.tensor, box 68 x 10 x 1 x 3 components starting at (x0 - 2, y0 - 1, z); cells outside the sample are
 // zero-filled by the copy engine) issued by one thread and completed on an mbarrier, instead of four cp.async per thread.
-// PLAIN = true: the forward-Euler stage with all four terms (terms == FE_TERM_ALL with E_elec, baseY == Y, no accumulator,
-// no folded stage combination, no raw-k output) -- the runtime switches of the epilogue become compile-time constants, which
-// frees the registers their pointers and flags hold and with them the per-plane recomputation of loop invariants.
-template <typename T, bool MAP, bool MIXED, bool TMA = false, bool PLAIN = false>
+// EPI != 0: a stage of forward Euler / Heun / classical RK4 with all four terms (terms == FE_TERM_ALL with E_elec, a stage
+// base, no folded stage combination, no raw-k output) -- the runtime switches of the epilogue become compile-time constants,
+// which frees the registers their pointers and flags hold and with them the per-plane recomputation of loop invariants:
+//   EPI 1: baseY == Y, no accumulator (Euler);  2: baseY == Y, accumulator (first stage of Heun / RK4);
+//   EPI 3: baseY != Y, no accumulator (last stage of Heun / RK4);  4: baseY != Y, accumulator (RK4 stages 2 and 3).
+// EPI 0 is the general epilogue (fe_rhs, AB3M2, RK45, partial term sets).
+template <typename T, bool MAP, bool MIXED, bool TMA = false, int EPI = 0>
 __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_constant__ CUtensorMap tmap)
 {
-    static_assert(!(PLAIN && MAP), "the plain variant has no material map");
+    constexpr bool PLAIN = EPI != 0;                 // specialised epilogue
+    constexpr bool BASEY = EPI == 1 || EPI == 2, ACC = EPI == 2 || EPI == 4;
+    static_assert(!(PLAIN && MAP), "the specialised epilogues have no material map");
     extern __shared__ __align__(128) unsigned char lsm[];
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
     // three planes ahead of their use; with a map the loader goes through registers (vacuum cells are zeroed).
@@ -565,11 +571,11 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             ex2 = (T)(mem.Eext[2] + mem.wamp[2] * wv);
     const uint32_t terms = PLAIN ? 15u : a.terms;
     const T* Ee = PLAIN || ((terms & 4u) && a.Eelec) ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
-    const T* base = PLAIN ? Y : a.baseY ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
-    const bool base_is_Y = PLAIN || a.baseY == a.Y;
+    const T* base = BASEY ? Y : (PLAIN || a.baseY) ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
+    const bool base_is_Y = BASEY || (!PLAIN && a.baseY == a.Y);
     T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
-    const T* ai = !PLAIN && a.accOut ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
-    T* ao = !PLAIN && a.accOut ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
+    const T* ai = (ACC || (!PLAIN && a.accOut)) ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
+    T* ao = (ACC || (!PLAIN && a.accOut)) ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
     const int nlin = PLAIN ? 0 : a.nlin;
     const LandauD<T> lc0 = smats[0];
     auto ldp = [](const T* q) { return *reinterpret_cast<const P2*>(q); };
@@ -724,7 +730,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             P2 bv = {0, 0};
-            if (base) {
+            if (PLAIN || base) {
                 // Euler: the stage base is the state itself, already in the tile (vacuum cells hold their raw value in memory)
                 if (base_is_Y && actA && actB) bv = pc[i];
                 else bv = ldp(base + i * N + r);
@@ -735,7 +741,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
                 bv = P2{bv.a + cj * lv.a, bv.b + cj * lv.b};
             }
             *reinterpret_cast<P2*>(Yout + i * N + r) = P2{bv.a + cy * kA[i], bv.b + cy * kB[i]};
-            if (ao) {
+            if (ACC || ao) {
                 const P2 av = ldp(ai + i * N + r);
                 *reinterpret_cast<P2*>(ao + i * N + r) = P2{av.a + ca * kA[i], av.b + ca * kB[i]};
             }
@@ -815,14 +821,22 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
         const int lim2 = 128 * 1024;
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        auto attr = [&](auto m, auto tm, auto ep) {
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(k_local2<T, false, decltype(m)::value, decltype(tm)::value, decltype(ep)::value>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        };
+        auto a2 = [&](auto m, auto tm) {
+            attr(m, tm, std::integral_constant<int, 0>{});
+            attr(m, tm, std::integral_constant<int, 1>{});
+            attr(m, tm, std::integral_constant<int, 2>{});
+            attr(m, tm, std::integral_constant<int, 3>{});
+            attr(m, tm, std::integral_constant<int, 4>{});
+        };
+        a2(std::true_type{}, std::true_type{});
+        a2(std::true_type{}, std::false_type{});
+        a2(std::false_type{}, std::true_type{});
+        a2(std::false_type{}, std::false_type{});
         if (e != cudaSuccess) return e;
         configured = 1;
     }
@@ -831,19 +845,23 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             if (a.mixed) k_local2<T, true, true><<<grid, 256, smem, st>>>(a, tmap);
             else k_local2<T, true, false><<<grid, 256, smem, st>>>(a, tmap);
         } else {
-            // forward-Euler stage with all four terms: the specialised epilogue (see k_local2)
-            const bool plain = a.terms == 15u && a.Eelec && a.baseY == a.Y && !a.accOut && !a.kOut && a.nlin == 0;
-            if (tma) {
-                if (plain) {
-                    if (a.mixed) k_local2<T, false, true, true, true><<<grid, 256, smem, st>>>(a, tmap);
-                    else k_local2<T, false, false, true, true><<<grid, 256, smem, st>>>(a, tmap);
-                } else if (a.mixed) k_local2<T, false, true, true><<<grid, 256, smem, st>>>(a, tmap);
-                else k_local2<T, false, false, true><<<grid, 256, smem, st>>>(a, tmap);
-            } else if (plain) {
-                if (a.mixed) k_local2<T, false, true, false, true><<<grid, 256, smem, st>>>(a, tmap);
-                else k_local2<T, false, false, false, true><<<grid, 256, smem, st>>>(a, tmap);
-            } else if (a.mixed) k_local2<T, false, true><<<grid, 256, smem, st>>>(a, tmap);
-            else k_local2<T, false, false><<<grid, 256, smem, st>>>(a, tmap);
+            // a stage of Euler / Heun / RK4 with all four terms: one of the specialised epilogues (see k_local2)
+            const bool spec = a.terms == 15u && a.Eelec && a.baseY && !a.kOut && a.nlin == 0;
+            const int epi = !spec ? 0 : a.baseY == a.Y ? (a.accOut ? 2 : 1) : (a.accOut ? 4 : 3);
+            auto go = [&](auto m, auto tm, auto ep) {
+                k_local2<T, false, decltype(m)::value, decltype(tm)::value, decltype(ep)::value><<<grid, 256, smem, st>>>(a, tmap);
+            };
+            auto d2 = [&](auto m, auto tm) {
+                switch (epi) {
+                    case 1: go(m, tm, std::integral_constant<int, 1>{}); break;
+                    case 2: go(m, tm, std::integral_constant<int, 2>{}); break;
+                    case 3: go(m, tm, std::integral_constant<int, 3>{}); break;
+                    case 4: go(m, tm, std::integral_constant<int, 4>{}); break;
+                    default: go(m, tm, std::integral_constant<int, 0>{}); break;
+                }
+            };
+            auto d1 = [&](auto m) { if (tma) d2(m, std::true_type{}); else d2(m, std::false_type{}); };
+            if (a.mixed) d1(std::true_type{}); else d1(std::false_type{});
         }
         return cudaGetLastError();
     }
