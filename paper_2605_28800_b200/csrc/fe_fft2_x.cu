@@ -335,6 +335,128 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// k6_xfwd: forward x pass without block barriers (fp64, Mc = 256, zero-padded rows, any spectrum layout).  As in k2_xfwd
+// the real rows of the block's next group are fetched into registers while the current group is transformed; as in
+// k6_xinv a row's 16 threads sit in one half-warp and own the row's 4 KB of shared memory, so the exchange of the
+// two-level transform (XOR swizzle within 128-byte pieces instead of a padding column), the natural-order copy and the
+// split step need __syncwarp only.  Half spectra leave by per-thread 16-byte stores straight from the split step.
+// ------------------------------------------------------------------------------------------------------------------
+template <typename T, int M>
+__global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T>* __restrict__ out, X2Args a)
+{
+    using C = XCfg<M>;
+    constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS;
+    static_assert(R1 == TPP && R2 == 16 && sizeof(cx<T>) == 16, "one second-step task per thread, 8 complex per 128-byte piece");
+    cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);   // w_M^(n2 k1) at [k1 * R2 + n2]
+    cx<T>* tws = tw + M;                              // w_2M^k, k < M
+    cx<T>* buf = tws + M;                             // [ROWS][M]
+    const int t = threadIdx.x, tp = t % TPP, rl = t / TPP;
+    cx<T>* rb = buf + rl * M;
+    constexpr int NLOAD = R1 / 2;
+    const int64_t ngroups = (a.nrows + ROWS - 1) / ROWS;
+    auto fetch = [&](int64_t grp, cx<T>* dst) {
+        const int64_t row = grp * ROWS + rl;
+        if (grp < ngroups && row < a.nrows) {
+            const cx<T>* src = reinterpret_cast<const cx<T>*>(in + row * a.real_rs) + tp;
+            static_for<NLOAD>([&](auto ic) {
+                constexpr int n1 = decltype(ic)::value;
+                dst[n1] = (tp + R2 * n1 < a.nc) ? src[R2 * n1] : cx<T>{0, 0};
+            });
+        } else {
+            static_for<NLOAD>([&](auto ic) { dst[decltype(ic)::value] = cx<T>{0, 0}; });
+        }
+    };
+    cx<T> vn[NLOAD];
+    fetch(blockIdx.x, vn);
+    {
+        const cx<T>* twg = static_cast<const cx<T>*>(a.tw);
+        for (int e = t; e < M; e += 256) {
+            tw[e] = twg[((e / R2) * (e % R2)) * (kTwiddleN / M)];
+            tws[e] = twg[e * (kTwiddleN / (2 * M))];
+        }
+    }
+    __syncthreads();
+    // exchange slot of element (k1, n2): k1 R2 + (n2 ^ (k1 & 7)); the thread-dependent part of both sides from eight bases
+    cx<T>* wb[8];       // write side, thread n2 = tp:  rb + (tp ^ c), + k1 R2 with c = k1 & 7
+    cx<T>* rd[8];       // read side, thread k1 = tp:   rb + tp R2 + (c ^ (tp & 7)), + 8 (n2 >> 3) with c = n2 & 7
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        wb[c] = rb + (tp ^ c);
+        rd[c] = rb + tp * R2 + (c ^ (tp & 7));
+    }
+    for (int64_t grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const int64_t row = grp * ROWS + rl;
+        const bool live = row < a.nrows;
+        cx<T> v[R1];
+        static_for<NLOAD>([&](auto ic) { v[decltype(ic)::value] = vn[decltype(ic)::value]; });
+        fetch(grp + gridDim.x, vn);
+        Dif<T, -1, R1, 0, true>::run(v);
+        __syncwarp();                       // the split step of the previous group has read the row
+        static_for<R1>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int k1 = brev<R1>(p);
+            cx<T> val = v[p];
+            if constexpr (k1 != 0) val = cmul(val, tw[k1 * R2 + tp]);
+            wb[k1 & 7][k1 * R2] = val;
+        });
+        __syncwarp();
+        cx<T> u[R2];
+        static_for<R2>([&](auto nc) {
+            constexpr int n = decltype(nc)::value;
+            u[n] = rd[n & 7][8 * (n >> 3)];
+        });
+        Dif<T, -1, R2>::run(u);
+        __syncwarp();                       // every thread of the row holds its exchange inputs
+        static_for<R2>([&](auto pc) {       // Z[k1 + R1 k2] in natural order
+            constexpr int p = decltype(pc)::value;
+            rb[tp + R1 * brev<R2>(p)] = u[p];
+        });
+        __syncwarp();
+        if (live) {
+            cx<T>* dst = out + spec_row(a, row);
+            for (int k = tp; k <= M / 2; k += TPP) {
+                const cx<T> Zk = rb[k], Zn = rb[(M - k) & (M - 1)];
+                const T ex = (T)0.5 * (Zk.x + Zn.x), ey = (T)0.5 * (Zk.y - Zn.y);
+                const T ox = (T)0.5 * (Zk.y + Zn.y), oy = (T)-0.5 * (Zk.x - Zn.x);
+                const cx<T> w = tws[k];
+                // X[k] = Xe + w Xo;  X[M-k] = conj(Xe) - conj(w Xo)   (w_2M^(M-k) = -conj(w_2M^k), Xo(M-k) = conj Xo(k))
+                const T px = ox * w.x - oy * w.y, py = ox * w.y + oy * w.x;
+                dst[spec_off(a, k)] = {ex + px, ey + py};
+                dst[spec_off(a, M - k)] = {ex - px, py - ey};
+            }
+        }
+    }
+}
+
+template <typename T>
+static bool try_launch_xfwd6(const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
+{
+    if constexpr (sizeof(T) != 8) {
+        return false;
+    } else {
+        constexpr int M = 256;
+        using C = XCfg<M>;
+        constexpr size_t smem = (size_t)(2 * M + C::ROWS * M) * sizeof(cx<T>);
+        static PerDevice<int> cache;
+        int& nblocks = cache.here();
+        if (!nblocks) {
+            cudaError_t e = cudaFuncSetAttribute(k6_xfwd<T, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            int dev = 0, sms = 0, per = 0;
+            if (e == cudaSuccess) e = cudaGetDevice(&dev);
+            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xfwd<T, M>, 256, smem);
+            if (e != cudaSuccess) { *err = e; return true; }
+            nblocks = sms * (per > 0 ? per : 1);
+        }
+        const int64_t ngroups = (a.nrows + C::ROWS - 1) / C::ROWS;
+        const int grid = (int)(ngroups < nblocks ? ngroups : nblocks);
+        k6_xfwd<T, M><<<grid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
+        *err = cudaGetLastError();
+        return true;
+    }
+}
+
 // tensor map of the tiled half spectra S1[plane][g][y][L] (as reals) with the box of one row group; false if unavailable
 template <typename T>
 static bool make_x_map(const void* S1, int ny, int G, int nplanes, int rows, CUtensorMap* map)
@@ -463,6 +585,10 @@ cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, in
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
     v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2};
+    if (M == 256 && prune) {
+        cudaError_t e = cudaSuccess;
+        if (v2::try_launch_xfwd6<T>(in, out, a, &e, st)) return e;
+    }
     return v2::launch_x<T, true>(M, prune, in, out, a, st);
 }
 
