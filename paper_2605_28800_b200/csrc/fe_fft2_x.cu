@@ -203,13 +203,13 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// k6_xinv: persistent inverse x pass for the tiled spectrum layout (fp64, Mc = 256).  The half spectra of a group of
-// ROWS rows ([g][row][L] in memory: one 3-D box) arrive by ONE tensor copy into a single shared-memory buffer; the rows
-// are transformed IN PLACE in that buffer: a row's R2 threads sit in one warp and own the row's 128-byte pieces, so the
-// exchange of the two-level transform needs only __syncwarp, and an XOR swizzle (column ^ (row of the exchange & 7))
-// replaces the padding column, which lets the 16 x 16 exchange fit into the 33 x 8 slots of the row.  As soon as every
-// thread holds its second-step inputs the buffer is free and thread 0 starts the copy of the block's next group, which
-// lands behind the second register FFT and the stores.
+// k6_xinv: persistent inverse x pass for the tiled spectrum layout (fp64, Mc = 256), no block barrier in its loop.  A warp
+// owns two rows of a group of ROWS rows: their half spectra ([g][row][L] in memory: a 3-D box of 2 rows) arrive by one
+// tensor copy on the warp's own mbarrier into the warp's own buffer and are transformed IN PLACE there: a row's R2 threads
+// own the row's 128-byte pieces, so the exchange of the two-level transform needs only __syncwarp, and an XOR swizzle
+// (column ^ (row of the exchange & 7)) replaces the padding column, which lets the 16 x 16 exchange fit into the 33 x 8
+// slots of the row.  As soon as every thread of the warp holds its second-step inputs the buffer is free and lane 0
+// starts the copy of the warp's rows of the block's next group, which lands behind the second register FFT and the stores.
 // ------------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned x6_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 
@@ -221,14 +221,16 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS, TWG = 8;
     constexpr int L = 128 / (int)sizeof(cx<T>);
     static_assert(R1 == TPP && L == 8, "one second-step task per thread, 8 complex per 128-byte piece");
-    cx<T>* buf = reinterpret_cast<cx<T>*>(fe2_smem);                       // [G][ROWS][L]
+    constexpr int WR = 32 / TPP;                                          // rows per warp
+    cx<T>* buf = reinterpret_cast<cx<T>*>(fe2_smem);                       // [warp][G][WR][L]
     cx<T>* tw = buf + (size_t)G * ROWS * L;                               // w_M^(n2 k1) at [k1 * R2 + n2]
     cx<T>* tws = tw + M;                                                  // w_2M^k
-    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tws + M);
-    const int t = threadIdx.x, tp = t % TPP, rl = t / TPP;
+    const int t = threadIdx.x, tp = t % TPP, rl = t / TPP, warp = t >> 5;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tws + M) + warp;     // the warp's mbarrier
+    cx<T>* wbuf = buf + (size_t)warp * G * WR * L;
     const int gpp = a.ny / ROWS;                                          // row groups per plane
     const int ngroups = nplanes * gpp;
-    const unsigned bytes = (unsigned)((size_t)G * ROWS * L * sizeof(cx<T>));
+    const unsigned bytes = (unsigned)((size_t)G * WR * L * sizeof(cx<T>));
     auto issue = [&](int grp) {
         int plane = grp / gpp;
         const int y0 = (grp - plane * gpp) * ROWS;
@@ -236,11 +238,11 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(x6_smem_u32(bar)), "r"(bytes) : "memory");
         asm volatile(
             "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];\n" ::"r"(
-                x6_smem_u32(buf)),
-            "l"(&imap), "r"(0), "r"(y0), "r"(0), "r"(plane), "r"(x6_smem_u32(bar))
+                x6_smem_u32(wbuf)),
+            "l"(&imap), "r"(0), "r"(y0 + WR * warp), "r"(0), "r"(plane), "r"(x6_smem_u32(bar))
             : "memory");
     };
-    if (t == 0) {
+    if ((t & 31) == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(x6_smem_u32(bar)));
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         if ((int)blockIdx.x < ngroups) issue(blockIdx.x);
@@ -254,7 +256,7 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     }
     __syncthreads();
     // element k of this thread's row / slot s of the row's in-place exchange
-    auto at = [&](int k) { return buf + ((k >> 3) * ROWS + rl) * L + (k & 7); };
+    auto at = [&](int k) { return wbuf + ((k >> 3) * WR + (rl % WR)) * L + (k & 7); };
     // the swizzled exchange addresses depend on the thread only through eight bases each (no shift / xor per access)
     static_assert(R2 == 2 * L, "two 128-byte pieces per exchange row");
     cx<T>* wb[8];       // element (tp ^ c) of the row's first piece: the write of exchange row o1 lands o1 * 2 pieces further
@@ -307,7 +309,7 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
                 constexpr int o1 = brev<R1>(p);
                 cx<T> val = v[p];
                 if constexpr (o1 != 0) val = cmulc(val, w[decltype(qc)::value]);
-                wb[o1 & 7][o1 * (R2 / L) * ROWS * L] = val;      // = *at(o1 * R2 + (tp ^ (o1 & 7)))
+                wb[o1 & 7][o1 * (R2 / L) * WR * L] = val;        // = *at(o1 * R2 + (tp ^ (o1 & 7)))
             });
         });
         __syncwarp();
@@ -315,10 +317,10 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
         cx<T> u[R2];
         static_for<R2>([&](auto nc) {                 // = *at(o1 * R2 + (n ^ (o1 & 7))), n = 8 (n >> 3) + (n & 7)
             constexpr int n = decltype(nc)::value;
-            u[n] = rbp[n & 7][(n >> 3) * ROWS * L];
+            u[n] = rbp[n & 7][(n >> 3) * WR * L];
         });
-        __syncthreads();                    // every row of the group is in registers: the buffer is free
-        if (t == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
+        __syncwarp();                       // both rows of the warp are in registers: the warp's buffer is free
+        if ((t & 31) == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
         Dif<T, +1, R2>::run(u);
         int plane = grp / gpp;
         const int y0 = (grp - plane * gpp) * ROWS;
@@ -501,8 +503,8 @@ static bool try_launch_xinv6(const void* in, void* out, const X2Args& a, cudaErr
         const int map_planes = a.pl_n ? nplanes / a.pl_n * a.pl_full : nplanes;
         CUtensorMap map;
         memset(&map, 0, sizeof(map));
-        if (!make_x_map<T>(in, a.ny, G, map_planes, C::ROWS, &map)) return false;
-        const size_t smem = (size_t)G * C::ROWS * L * sizeof(cx<T>) + (size_t)2 * M * sizeof(cx<T>) + 16;
+        if (!make_x_map<T>(in, a.ny, G, map_planes, 32 / C::TPP, &map)) return false;       // one box = the two rows of a warp
+        const size_t smem = (size_t)G * C::ROWS * L * sizeof(cx<T>) + (size_t)2 * M * sizeof(cx<T>) + 8 * 8;
         if (smem > 113 * 1024) return false;
         static PerDevice<int> cache;
         int& nblocks = cache.here();
