@@ -301,7 +301,7 @@ def run_cuda(args):
     cdom = ctr.get(dom) if isinstance(ctr.get(dom), dict) else {}
     traffic = cdom.get("dram_bytes") if cdom else (ctr.get(dom) if not isinstance(ctr.get(dom), dict) else None)
     # kernel that serves the profile slot on the size-specialised path (every bench workload but cfg1 takes it)
-    fast_names = {"xfwd": "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>",
+    fast_names = {"xfwd": "k6_xfwd" if (args.dtype == "f64" and int(w.n[0]) == 256) else "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>",
                   "xinv": "k6_xinv" if (args.dtype == "f64" and int(w.n[0]) == 256) else "k2_xinv",
                   "local": "k_local2", "xyfwd": "k_xyfwd", "xyinv": "k_xyinv"}
     generic = args.workload == "cfg1"

@@ -348,6 +348,10 @@ __device__ __forceinline__ void l_mbar_expect_tx(void* bar, unsigned bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(lsm_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void l_mbar_arrive(void* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(lsm_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void l_mbar_wait(void* bar, unsigned parity)
 {
     const unsigned addr = lsm_u32(bar);
@@ -396,7 +400,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     extern __shared__ __align__(128) unsigned char lsm[];
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
     // three planes ahead of their use; with a map the loader goes through registers (vacuum cells are zeroed).
-    constexpr int NS = MAP ? 4 : 5;
+    constexpr int NS = MAP ? 4 : TMA ? 6 : 5;
     constexpr int SLOT = (int)(k2_slot_bytes<T>() / sizeof(T));             // elements between two plane slots
     static_assert(!(TMA && MAP), "the tensor-copy loader has no vacuum masking");
     T* tiles = reinterpret_cast<T*>(lsm);                                   // [NS][SLOT >= 3 k2Tile]
@@ -404,7 +408,8 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + NS * k2Tile);  // [nmat]
     unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(
-        lsm + (((size_t)(sact + a.nmat - lsm) + 7) / 8) * 8);                // [NS] mbarriers of the tensor-copy loader
+        lsm + (((size_t)(sact + a.nmat - lsm) + 7) / 8) * 8);                // [NS] "plane has landed" mbarriers of the tensor-copy loader
+    unsigned long long* ebars = bars + NS;                                   // [NS] "every warp is done with the plane" mbarriers
     using P2 = pair_t<T>;
 
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
@@ -530,7 +535,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     };
     auto tma_wait = [&](int z) { l_mbar_wait(&bars[slot_of(z)], (unsigned)(((z - z0 + 1) / NS) & 1)); };
     if (TMA && t == 0) {
-        for (int i = 0; i < NS; ++i) l_mbar_init(&bars[i], 1);
+        for (int i = 0; i < NS; ++i) { l_mbar_init(&bars[i], 1); l_mbar_init(&ebars[i], 8); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();          // coefficient tables visible (fetch_plane reads sact); mbarriers initialised
@@ -596,6 +601,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     // slots of planes z-1, z, z+1 and the phase bits of the slots' mbarriers, carried from plane to plane (no division per plane)
     int sm1 = 0, s00 = 1, sp1 = 2;
     unsigned phases = 3u;                            // slots 0 and 1 were awaited once in the prologue
+    unsigned ephases = 0u;                           // thread 0: phase bits of the release mbarriers
     int64_t r = (int64_t)z0 * nxy + rxy;             // cell pair (x, y, z) of this thread
     for (int z = z0; z < z1; ++z, r += nxy, sm1 = s00, s00 = sp1, sp1 = (sp1 + 1 == NS ? 0 : sp1 + 1)) {
         if (MAP) {
@@ -603,11 +609,20 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             __syncthreads();
             if (z + 1 < z1) fetch_plane(z + 2);      // in flight while plane z is computed
         } else if (TMA) {
+            // no block barrier: a warp releases plane z-2 (last read in its iteration z-1) on the slot's second mbarrier,
+            // and thread 0 refills the slot of plane z-3 once all eight warps have released it
+            if (z > z0) {
+                __syncwarp();
+                if ((t & 31) == 0) l_mbar_arrive(&ebars[sm1 == 0 ? NS - 1 : sm1 - 1]);
+            }
             l_mbar_wait(&bars[sp1], (phases >> sp1) & 1u);   // planes <= z+1 have landed
             phases ^= 1u << sp1;
-            __syncthreads();                                 // every thread is done with plane z-2
-            if (t == 0 && z + 3 <= z1) {                     // plane z+3 into the slot of plane z-2
+            if (t == 0 && z + 3 <= z1) {                     // plane z+3 into the slot of plane z-3
                 const int s3 = sp1 + 2 >= NS ? sp1 + 2 - NS : sp1 + 2;
+                if (z - z0 >= 2) {                           // (the first NS planes find their slots fresh)
+                    l_mbar_wait(&ebars[s3], (ephases >> s3) & 1u);
+                    ephases ^= 1u << s3;
+                }
                 l_mbar_expect_tx(&bars[s3], (unsigned)(3 * k2Tile * sizeof(T)));
                 l_tma_load_4d(tiles + s3 * SLOT, &tmap, x0 - 2, y0 - 1, z + 3, 3 * b, &bars[s3]);
             }
@@ -803,13 +818,13 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     while (zc > 8 && (int64_t)ntx * nty * ((nzl + zc - 1) / zc) * a.batch < 12 * 148) zc = (zc + 1) / 2;
     a.zchunk = zc;
     dim3 grid(ntx * nty, (nzl + zc - 1) / zc, a.batch);
-    const int ns = a.map ? 4 : 5;         // ring slots of k_local2
-    const size_t smem = two ? (size_t)ns * k2_slot_bytes<T>() + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1) + 8 + ns * 8
-                            : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
     // halo planes by tensor copy (zero fill outside the sample) when there is neither a material map nor a periodic axis
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
     const bool tma = two && !a.map && !(a.periodic[0] | a.periodic[1] | a.periodic[2]) && make_state_map<T>(a, &tmap);
+    const int ns = a.map ? 4 : tma ? 6 : 5;         // ring slots of k_local2
+    const size_t smem = two ? (size_t)ns * k2_slot_bytes<T>() + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1) + 8 + 2 * ns * 8
+                            : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
     static PerDevice<int> cache;
     int& configured = cache.here();
     if (!configured) {
