@@ -203,8 +203,8 @@ __global__ void __launch_bounds__(256, M >= 512 ? 1 : 2) k2_xinv(const cx<T>* __
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// k6_xinv: persistent inverse x pass for the tiled spectrum layout (fp64, Mc = 256), no block barrier in its loop.  A warp
-// owns two rows of a group of ROWS rows: their half spectra ([g][row][L] in memory: a 3-D box of 2 rows) arrive by one
+// k6_xinv: persistent inverse x pass for the tiled spectrum layout (Mc = R2 * R2: 256 in fp64 / fp32, 64 in fp64), no block
+// barrier in its loop.  A warp owns 32 / R2 rows of a group of ROWS rows (two at Mc = 256, described here): their half spectra ([g][row][L] in memory: a 3-D box of 2 rows) arrive by one
 // tensor copy on the warp's own mbarrier into the warp's own buffer and are transformed IN PLACE there: a row's R2 threads
 // own the row's 128-byte pieces, so the exchange of the two-level transform needs only __syncwarp, and an XOR swizzle
 // (column ^ (row of the exchange & 7)) replaces the padding column, which lets the 16 x 16 exchange fit into the 33 x 8
@@ -219,8 +219,9 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
 {
     using C = XCfg<M>;
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS, TWG = 8;
-    constexpr int L = 128 / (int)sizeof(cx<T>);
-    static_assert(R1 == TPP && L == 8, "one second-step task per thread, 8 complex per 128-byte piece");
+    constexpr int L = 128 / (int)sizeof(cx<T>);                           // complex per 128-byte piece
+    constexpr int SW = R2 < L ? R2 : L;                                   // the swizzle permutes within pieces
+    static_assert(R1 == TPP && R2 % L == 0, "one second-step task per thread; an exchange row is whole pieces");
     constexpr int WR = 32 / TPP;                                          // rows per warp
     cx<T>* buf = reinterpret_cast<cx<T>*>(fe2_smem);                       // [warp][G][WR][L]
     cx<T>* tw = buf + (size_t)G * ROWS * L;                               // w_M^(n2 k1) at [k1 * R2 + n2]
@@ -256,13 +257,14 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     }
     __syncthreads();
     // element k of this thread's row / slot s of the row's in-place exchange
-    auto at = [&](int k) { return wbuf + ((k >> 3) * WR + (rl % WR)) * L + (k & 7); };
-    // the swizzled exchange addresses depend on the thread only through eight bases each (no shift / xor per access)
-    static_assert(R2 == 2 * L, "two 128-byte pieces per exchange row");
-    cx<T>* wb[8];       // element (tp ^ c) of the row's first piece: the write of exchange row o1 lands o1 * 2 pieces further
-    cx<T>* rbp[8];      // element ((n & 7) ^ (tp & 7)) of exchange row tp: the read of column n adds its piece (n >> 3)
+    auto at = [&](int k) { return wbuf + ((k / L) * WR + (rl % WR)) * L + (k % L); };
+    // with eight-element pieces the swizzled exchange addresses depend on the thread only through eight bases each (no
+    // shift / xor per access); otherwise they are formed per access
+    constexpr int NB = SW == 8 ? 8 : 1;
+    cx<T>* wb[NB];      // element (tp ^ c) of the row's first pieces: the write of exchange row o1 lands o1 * R2 / L pieces further
+    cx<T>* rbp[NB];     // element ((n & 7) ^ (tp & 7)) of exchange row tp: the read of column n adds its piece (n >> 3)
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
+    for (int c = 0; c < NB; ++c) {
         wb[c] = at(tp ^ c);
         rbp[c] = at(tp * R2 + (c ^ (tp & 7)));
     }
@@ -309,7 +311,8 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
                 constexpr int o1 = brev<R1>(p);
                 cx<T> val = v[p];
                 if constexpr (o1 != 0) val = cmulc(val, w[decltype(qc)::value]);
-                wb[o1 & 7][o1 * (R2 / L) * WR * L] = val;        // = *at(o1 * R2 + (tp ^ (o1 & 7)))
+                if constexpr (SW == 8) wb[o1 & 7][o1 * (R2 / L) * WR * L] = val;        // = *at(o1 * R2 + (tp ^ (o1 & 7)))
+                else *at(o1 * R2 + (tp ^ (o1 & (SW - 1)))) = val;
             });
         });
         __syncwarp();
@@ -317,7 +320,8 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
         cx<T> u[R2];
         static_for<R2>([&](auto nc) {                 // = *at(o1 * R2 + (n ^ (o1 & 7))), n = 8 (n >> 3) + (n & 7)
             constexpr int n = decltype(nc)::value;
-            u[n] = rbp[n & 7][(n >> 3) * WR * L];
+            if constexpr (SW == 8) u[n] = rbp[n & 7][(n >> 3) * WR * L];
+            else u[n] = *at(o1 * R2 + (n ^ (o1 & (SW - 1))));
         });
         __syncwarp();                       // both rows of the warp are in registers: the warp's buffer is free
         if ((t & 31) == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
@@ -338,18 +342,20 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// k6_xfwd: forward x pass without block barriers (fp64, Mc = 256, zero-padded rows, any spectrum layout).  As in k2_xfwd
-// the real rows of the block's next group are fetched into registers while the current group is transformed; as in
-// k6_xinv a row's 16 threads sit in one half-warp and own the row's 4 KB of shared memory, so the exchange of the
-// two-level transform (XOR swizzle within 128-byte pieces instead of a padding column), the natural-order copy and the
-// split step need __syncwarp only.  Half spectra leave by per-thread 16-byte stores straight from the split step.
+// k6_xfwd: forward x pass without block barriers (Mc = R2 * R2: 256 in fp64 / fp32, 64 in fp64; zero-padded rows, any
+// spectrum layout).  As in k2_xfwd the real rows of the block's next group are fetched into registers while the current
+// group is transformed; as in k6_xinv a row's R2 threads sit in one warp and own the row's shared memory, so the exchange
+// of the two-level transform (XOR swizzle within 128-byte pieces instead of a padding column), the natural-order copy and
+// the split step need __syncwarp only.  Half spectra leave by per-thread stores straight from the split step.
 // ------------------------------------------------------------------------------------------------------------------
 template <typename T, int M>
 __global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T>* __restrict__ out, X2Args a)
 {
     using C = XCfg<M>;
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS;
-    static_assert(R1 == TPP && R2 == 16 && sizeof(cx<T>) == 16, "one second-step task per thread, 8 complex per 128-byte piece");
+    constexpr int L = 128 / (int)sizeof(cx<T>);       // complex per 128-byte piece
+    constexpr int SW = R2 < L ? R2 : L;               // the swizzle permutes within pieces (or within an exchange row)
+    static_assert(R1 == TPP && R2 * (int)sizeof(cx<T>) >= 128, "one second-step task per thread; an exchange row is whole pieces");
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);   // w_M^(n2 k1) at [k1 * R2 + n2]
     cx<T>* tws = tw + M;                              // w_2M^k, k < M
     cx<T>* buf = tws + M;                             // [ROWS][M]
@@ -379,11 +385,13 @@ __global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T
         }
     }
     __syncthreads();
-    // exchange slot of element (k1, n2): k1 R2 + (n2 ^ (k1 & 7)); the thread-dependent part of both sides from eight bases
-    cx<T>* wb[8];       // write side, thread n2 = tp:  rb + (tp ^ c), + k1 R2 with c = k1 & 7
-    cx<T>* rd[8];       // read side, thread k1 = tp:   rb + tp R2 + (c ^ (tp & 7)), + 8 (n2 >> 3) with c = n2 & 7
+    // exchange slot of element (k1, n2): k1 R2 + (n2 ^ (k1 & (SW - 1))).  With eight-element pieces the thread-dependent part
+    // of both sides comes from eight bases; otherwise the addresses are formed per access
+    constexpr int NB = SW == 8 ? 8 : 1;
+    cx<T>* wb[NB];      // write side, thread n2 = tp:  rb + (tp ^ c), + k1 R2 with c = k1 & 7
+    cx<T>* rd[NB];      // read side, thread k1 = tp:   rb + tp R2 + (c ^ (tp & 7)), + 8 (n2 >> 3) with c = n2 & 7
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
+    for (int c = 0; c < NB; ++c) {
         wb[c] = rb + (tp ^ c);
         rd[c] = rb + tp * R2 + (c ^ (tp & 7));
     }
@@ -400,13 +408,15 @@ __global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T
             constexpr int k1 = brev<R1>(p);
             cx<T> val = v[p];
             if constexpr (k1 != 0) val = cmul(val, tw[k1 * R2 + tp]);
-            wb[k1 & 7][k1 * R2] = val;
+            if constexpr (SW == 8) wb[k1 & 7][k1 * R2] = val;
+            else rb[k1 * R2 + (tp ^ (k1 & (SW - 1)))] = val;
         });
         __syncwarp();
         cx<T> u[R2];
         static_for<R2>([&](auto nc) {
             constexpr int n = decltype(nc)::value;
-            u[n] = rd[n & 7][8 * (n >> 3)];
+            if constexpr (SW == 8) u[n] = rd[n & 7][8 * (n >> 3)];
+            else u[n] = rb[tp * R2 + (n ^ (tp & (SW - 1)))];
         });
         Dif<T, -1, R2>::run(u);
         __syncwarp();                       // every thread of the row holds its exchange inputs
@@ -431,32 +441,43 @@ __global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T
     }
 }
 
-template <typename T>
-static bool try_launch_xfwd6(const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
+template <typename T, int M>
+static cudaError_t launch_xfwd6(const void* in, void* out, const X2Args& a, cudaStream_t st)
 {
-    if constexpr (sizeof(T) != 8) {
-        return false;
-    } else {
-        constexpr int M = 256;
-        using C = XCfg<M>;
-        constexpr size_t smem = (size_t)(2 * M + C::ROWS * M) * sizeof(cx<T>);
-        static PerDevice<int> cache;
-        int& nblocks = cache.here();
-        if (!nblocks) {
-            cudaError_t e = cudaFuncSetAttribute(k6_xfwd<T, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            int dev = 0, sms = 0, per = 0;
-            if (e == cudaSuccess) e = cudaGetDevice(&dev);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xfwd<T, M>, 256, smem);
-            if (e != cudaSuccess) { *err = e; return true; }
-            nblocks = sms * (per > 0 ? per : 1);
-        }
-        const int64_t ngroups = (a.nrows + C::ROWS - 1) / C::ROWS;
-        const int grid = (int)(ngroups < nblocks ? ngroups : nblocks);
-        k6_xfwd<T, M><<<grid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
-        *err = cudaGetLastError();
+    using C = XCfg<M>;
+    constexpr size_t smem = (size_t)(2 * M + C::ROWS * M) * sizeof(cx<T>);
+    static PerDevice<int> cache;
+    int& nblocks = cache.here();
+    if (!nblocks) {
+        cudaError_t e = cudaFuncSetAttribute(k6_xfwd<T, M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        int dev = 0, sms = 0, per = 0;
+        if (e == cudaSuccess) e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xfwd<T, M>, 256, smem);
+        if (e != cudaSuccess) return e;
+        nblocks = sms * (per > 0 ? per : 1);
+    }
+    const int64_t ngroups = (a.nrows + C::ROWS - 1) / C::ROWS;
+    const int grid = (int)(ngroups < nblocks ? ngroups : nblocks);
+    k6_xfwd<T, M><<<grid, 256, smem, st>>>(static_cast<const T*>(in), static_cast<cx<T>*>(out), a);
+    return cudaGetLastError();
+}
+
+// the barrier-free forward pass exists for Mc = 256 (fp64, fp32) and Mc = 64 (fp64), zero-padded rows
+template <typename T>
+static bool try_launch_xfwd6(int M, const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
+{
+    if (M == 256) {
+        *err = launch_xfwd6<T, 256>(in, out, a, st);
         return true;
     }
+    if constexpr (sizeof(T) == 8) {
+        if (M == 64) {
+            *err = launch_xfwd6<T, 64>(in, out, a, st);
+            return true;
+        }
+    }
+    return false;
 }
 
 // tensor map of the tiled half spectra S1[plane][g][y][L] (as reals) with the box of one row group; false if unavailable
@@ -486,43 +507,52 @@ static bool make_x_map(const void* S1, int ny, int G, int nplanes, int rows, CUt
                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// persistent tensor-copy inverse pass when the layout is the tiled one (fp64, Mc = 256, whole row groups per plane)
-template <typename T, bool PRUNE>
-static bool try_launch_xinv6(const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
+// persistent tensor-copy inverse pass when the layout is the tiled one (whole row groups per plane): Mc = 256 (fp64, fp32)
+// and Mc = 64 (fp64)
+template <typename T, int M, bool PRUNE>
+static bool launch_xinv6(const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
 {
-    if constexpr (sizeof(T) != 8) {
-        return false;
-    } else {
-        constexpr int M = 256;
-        using C = XCfg<M>;
-        constexpr int L = 8;
-        if (a.lg != 3 || a.s_row != L || a.s_g != (int64_t)a.ny * L || a.ny % C::ROWS || a.s_plane % ((int64_t)a.ny * L)) return false;
-        const int G = (int)(a.s_plane / ((int64_t)a.ny * L));
-        if (a.nrows % a.ny) return false;
-        const int nplanes = (int)(a.nrows / a.ny);
-        const int map_planes = a.pl_n ? nplanes / a.pl_n * a.pl_full : nplanes;
-        CUtensorMap map;
-        memset(&map, 0, sizeof(map));
-        if (!make_x_map<T>(in, a.ny, G, map_planes, 32 / C::TPP, &map)) return false;       // one box = the two rows of a warp
-        const size_t smem = (size_t)G * C::ROWS * L * sizeof(cx<T>) + (size_t)2 * M * sizeof(cx<T>) + 8 * 8;
-        if (smem > 113 * 1024) return false;
-        static PerDevice<int> cache;
-        int& nblocks = cache.here();
-        if (!nblocks) {
-            cudaError_t e = cudaFuncSetAttribute(k6_xinv<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
-            int dev = 0, sms = 0, per = 0;
-            if (e == cudaSuccess) e = cudaGetDevice(&dev);
-            if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-            if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xinv<T, M, PRUNE>, 256, smem);
-            if (e != cudaSuccess) { *err = e; return true; }
-            nblocks = sms * (per > 0 ? per : 1);
-        }
-        const int ngroups = nplanes * (a.ny / C::ROWS);
-        const int grid = ngroups < nblocks ? ngroups : nblocks;
-        k6_xinv<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<T*>(out), a, G, nplanes, map);
-        *err = cudaGetLastError();
-        return true;
+    using C = XCfg<M>;
+    constexpr int L = 128 / (int)sizeof(cx<T>);
+    int lgL = 0;
+    while ((1 << lgL) < L) ++lgL;
+    if (a.lg != lgL || a.s_row != L || a.s_g != (int64_t)a.ny * L || a.ny % C::ROWS || a.s_plane % ((int64_t)a.ny * L)) return false;
+    const int G = (int)(a.s_plane / ((int64_t)a.ny * L));
+    if (a.nrows % a.ny || G * L < M + 1) return false;
+    const int nplanes = (int)(a.nrows / a.ny);
+    const int map_planes = a.pl_n ? nplanes / a.pl_n * a.pl_full : nplanes;
+    CUtensorMap map;
+    memset(&map, 0, sizeof(map));
+    if (!make_x_map<T>(in, a.ny, G, map_planes, 32 / C::TPP, &map)) return false;       // one box = the rows of a warp
+    const size_t smem = (size_t)G * C::ROWS * L * sizeof(cx<T>) + (size_t)2 * M * sizeof(cx<T>) + 8 * 8;
+    if (smem > 113 * 1024) return false;
+    static PerDevice<int> cache;
+    int& sms = cache.here();
+    if (!sms) {
+        cudaError_t e = cudaFuncSetAttribute(k6_xinv<T, M, PRUNE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
+        int dev = 0;
+        if (e == cudaSuccess) e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) { sms = 0; *err = e; return true; }
     }
+    int per = 0;        // the shared-memory size depends on the layout (G): ask every time (a cheap host-side query)
+    if ((*err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xinv<T, M, PRUNE>, 256, smem)) != cudaSuccess) return true;
+    const int nblocks = sms * (per > 0 ? per : 1);
+    const int ngroups = nplanes * (a.ny / C::ROWS);
+    const int grid = ngroups < nblocks ? ngroups : nblocks;
+    k6_xinv<T, M, PRUNE><<<grid, 256, smem, st>>>(static_cast<T*>(out), a, G, nplanes, map);
+    *err = cudaGetLastError();
+    return true;
+}
+
+template <typename T, bool PRUNE>
+static bool try_launch_xinv6(int M, const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
+{
+    if (M == 256) return launch_xinv6<T, 256, PRUNE>(in, out, a, err, st);
+    if constexpr (sizeof(T) == 8) {
+        if (M == 64) return launch_xinv6<T, 64, PRUNE>(in, out, a, err, st);
+    }
+    return false;
 }
 
 template <typename T, int M, bool PRUNE, bool FWD>
@@ -587,9 +617,9 @@ cudaError_t launch_xfwd2(const FftCtx& c, const T* in, void* out, int n_real, in
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
     v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2};
-    if (M == 256 && prune) {
+    if (prune) {
         cudaError_t e = cudaSuccess;
-        if (v2::try_launch_xfwd6<T>(in, out, a, &e, st)) return e;
+        if (v2::try_launch_xfwd6<T>(M, in, out, a, &e, st)) return e;
     }
     return v2::launch_x<T, true>(M, prune, in, out, a, st);
 }
@@ -604,9 +634,9 @@ cudaError_t launch_xinv2(const FftCtx& c, const void* in, T* out, int n_real, in
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
     v2::X2Args a{c.tw, nrows, real_rs, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2};
-    if (M == 256 && prune) {
+    if (prune) {
         cudaError_t e = cudaSuccess;
-        if (v2::try_launch_xinv6<T, true>(in, out, a, &e, st)) return e;
+        if (v2::try_launch_xinv6<T, true>(M, in, out, a, &e, st)) return e;
     }
     return v2::launch_x<T, false>(M, prune, in, out, a, st);
 }
@@ -618,12 +648,12 @@ cudaError_t launch_xinv2_slab(const FftCtx& c, const void* in, T* out, int n_rea
                               const int64_t spec[4], int lanes, cudaStream_t st)
 {
     const int M = c.plan[0].M;
-    if (M != 256 || n_real > M || (n_real & 1)) return cudaErrorNotSupported;
+    if ((M != 256 && M != 64) || n_real > M || (n_real & 1)) return cudaErrorNotSupported;
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
     v2::X2Args a{c.tw, (int64_t)comps * zn * ny, n_real, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2, zn, nz, zb};
     cudaError_t e = cudaSuccess;
-    if (v2::try_launch_xinv6<T, true>(in, out, a, &e, st)) return e;
+    if (v2::try_launch_xinv6<T, true>(M, in, out, a, &e, st)) return e;
     return cudaErrorNotSupported;
 }
 bool xinv_slab_supported(int Mc, int n_real, int ny, int lanes, size_t elem) { return elem == 8 && Mc == 256 && n_real <= Mc && ny % 16 == 0 && lanes == 8; }
