@@ -221,7 +221,8 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS, TWG = 8;
     constexpr int L = 128 / (int)sizeof(cx<T>);                           // complex per 128-byte piece
     constexpr int SW = R2 < L ? R2 : L;                                   // the swizzle permutes within pieces
-    static_assert(R1 == TPP && R2 % L == 0, "one second-step task per thread; an exchange row is whole pieces");
+    constexpr int NT3 = R1 / TPP;                                         // second-step tasks (exchange rows tp + it TPP) per thread
+    static_assert(R1 % TPP == 0 && R2 % L == 0 && (NT3 == 1 || TPP % 8 == 0), "an exchange row is whole pieces");
     constexpr int WR = 32 / TPP;                                          // rows per warp
     cx<T>* buf = reinterpret_cast<cx<T>*>(fe2_smem);                       // [warp][G][WR][L]
     cx<T>* tw = buf + (size_t)G * ROWS * L;                               // w_M^(n2 k1) at [k1 * R2 + n2]
@@ -316,27 +317,34 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
             });
         });
         __syncwarp();
-        const int o1 = tp;
-        cx<T> u[R2];
-        static_for<R2>([&](auto nc) {                 // = *at(o1 * R2 + (n ^ (o1 & 7))), n = 8 (n >> 3) + (n & 7)
-            constexpr int n = decltype(nc)::value;
-            if constexpr (SW == 8) u[n] = rbp[n & 7][(n >> 3) * WR * L];
-            else u[n] = *at(o1 * R2 + (n ^ (o1 & (SW - 1))));
+        cx<T> u[NT3][R2];
+        static_for<NT3>([&](auto tc) {
+            constexpr int it = decltype(tc)::value;
+            const int o1 = tp + it * TPP;
+            static_for<R2>([&](auto nc) {             // = *at(o1 * R2 + (n ^ (o1 & 7))), n = 8 (n >> 3) + (n & 7)
+                constexpr int n = decltype(nc)::value;
+                if constexpr (SW == 8) u[it][n] = rbp[n & 7][((n >> 3) + it * (TPP * R2 / L)) * WR * L];    // (tp + it TPP) & 7 == tp & 7
+                else u[it][n] = *at(o1 * R2 + (n ^ (o1 & (SW - 1))));
+            });
         });
-        __syncwarp();                       // both rows of the warp are in registers: the warp's buffer is free
+        __syncwarp();                       // the rows of the warp are in registers: the warp's buffer is free
         if ((t & 31) == 0 && grp + (int)gridDim.x < ngroups) issue(grp + gridDim.x);
-        Dif<T, +1, R2>::run(u);
         int plane = grp / gpp;
         const int y0 = (grp - plane * gpp) * ROWS;
         if (a.pl_n) plane = (plane / a.pl_n) * a.pl_full + plane % a.pl_n;
         const int64_t row = (int64_t)plane * a.ny + y0 + rl;
-        cx<T>* dst = reinterpret_cast<cx<T>*>(out + row * a.real_rs) + o1;
-        static_for<R2>([&](auto pc) {
-            constexpr int p = decltype(pc)::value;
-            constexpr int o2 = brev<R2>(p);
-            if constexpr (!PRUNE || o2 < R2 / 2) {
-                if (!PRUNE || o1 + R1 * o2 < a.nc) dst[R1 * o2] = u[p];
-            }
+        static_for<NT3>([&](auto tc) {
+            constexpr int it = decltype(tc)::value;
+            const int o1 = tp + it * TPP;
+            Dif<T, +1, R2>::run(u[it]);
+            cx<T>* dst = reinterpret_cast<cx<T>*>(out + row * a.real_rs) + o1;
+            static_for<R2>([&](auto pc) {
+                constexpr int p = decltype(pc)::value;
+                constexpr int o2 = brev<R2>(p);
+                if constexpr (!PRUNE || o2 < R2 / 2) {
+                    if (!PRUNE || o1 + R1 * o2 < a.nc) dst[R1 * o2] = u[it][p];
+                }
+            });
         });
     }
 }
@@ -355,7 +363,8 @@ __global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T
     constexpr int R1 = C::R1, R2 = C::R2, TPP = C::TPP, ROWS = C::ROWS;
     constexpr int L = 128 / (int)sizeof(cx<T>);       // complex per 128-byte piece
     constexpr int SW = R2 < L ? R2 : L;               // the swizzle permutes within pieces (or within an exchange row)
-    static_assert(R1 == TPP && R2 * (int)sizeof(cx<T>) >= 128, "one second-step task per thread; an exchange row is whole pieces");
+    constexpr int NT3 = R1 / TPP;                     // second-step tasks (rows k1 = tp + it TPP of the exchange) per thread
+    static_assert(R1 % TPP == 0 && R2 * (int)sizeof(cx<T>) >= 128 && (NT3 == 1 || TPP % 8 == 0), "an exchange row is whole pieces");
     cx<T>* tw = reinterpret_cast<cx<T>*>(fe2_smem);   // w_M^(n2 k1) at [k1 * R2 + n2]
     cx<T>* tws = tw + M;                              // w_2M^k, k < M
     cx<T>* buf = tws + M;                             // [ROWS][M]
@@ -412,17 +421,23 @@ __global__ void __launch_bounds__(256, 2) k6_xfwd(const T* __restrict__ in, cx<T
             else rb[k1 * R2 + (tp ^ (k1 & (SW - 1)))] = val;
         });
         __syncwarp();
-        cx<T> u[R2];
-        static_for<R2>([&](auto nc) {
-            constexpr int n = decltype(nc)::value;
-            if constexpr (SW == 8) u[n] = rd[n & 7][8 * (n >> 3)];
-            else u[n] = rb[tp * R2 + (n ^ (tp & (SW - 1)))];
+        cx<T> u[NT3][R2];
+        static_for<NT3>([&](auto tc) {
+            constexpr int it = decltype(tc)::value;
+            static_for<R2>([&](auto nc) {
+                constexpr int n = decltype(nc)::value;
+                if constexpr (SW == 8) u[it][n] = rd[n & 7][8 * (n >> 3) + it * TPP * R2];     // (tp + it TPP) & 7 == tp & 7
+                else u[it][n] = rb[(tp + it * TPP) * R2 + (n ^ ((tp + it * TPP) & (SW - 1)))];
+            });
+            Dif<T, -1, R2>::run(u[it]);
         });
-        Dif<T, -1, R2>::run(u);
         __syncwarp();                       // every thread of the row holds its exchange inputs
-        static_for<R2>([&](auto pc) {       // Z[k1 + R1 k2] in natural order
-            constexpr int p = decltype(pc)::value;
-            rb[tp + R1 * brev<R2>(p)] = u[p];
+        static_for<NT3>([&](auto tc) {      // Z[k1 + R1 k2] in natural order
+            constexpr int it = decltype(tc)::value;
+            static_for<R2>([&](auto pc) {
+                constexpr int p = decltype(pc)::value;
+                rb[tp + it * TPP + R1 * brev<R2>(p)] = u[it][p];
+            });
         });
         __syncwarp();
         if (live) {
@@ -463,7 +478,7 @@ static cudaError_t launch_xfwd6(const void* in, void* out, const X2Args& a, cuda
     return cudaGetLastError();
 }
 
-// the barrier-free forward pass exists for Mc = 256 (fp64, fp32) and Mc = 64 (fp64), zero-padded rows
+// the barrier-free forward pass exists for Mc = 256 (fp64, fp32) and Mc = 128, 64 (fp64), zero-padded rows
 template <typename T>
 static bool try_launch_xfwd6(int M, const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
 {
@@ -474,6 +489,10 @@ static bool try_launch_xfwd6(int M, const void* in, void* out, const X2Args& a, 
     if constexpr (sizeof(T) == 8) {
         if (M == 64) {
             *err = launch_xfwd6<T, 64>(in, out, a, st);
+            return true;
+        }
+        if (M == 128) {
+            *err = launch_xfwd6<T, 128>(in, out, a, st);
             return true;
         }
     }
@@ -508,7 +527,7 @@ static bool make_x_map(const void* S1, int ny, int G, int nplanes, int rows, CUt
 }
 
 // persistent tensor-copy inverse pass when the layout is the tiled one (whole row groups per plane): Mc = 256 (fp64, fp32)
-// and Mc = 64 (fp64)
+// and Mc = 128, 64 (fp64)
 template <typename T, int M, bool PRUNE>
 static bool launch_xinv6(const void* in, void* out, const X2Args& a, cudaError_t* err, cudaStream_t st)
 {
@@ -551,6 +570,7 @@ static bool try_launch_xinv6(int M, const void* in, void* out, const X2Args& a, 
     if (M == 256) return launch_xinv6<T, 256, PRUNE>(in, out, a, err, st);
     if constexpr (sizeof(T) == 8) {
         if (M == 64) return launch_xinv6<T, 64, PRUNE>(in, out, a, err, st);
+        if (M == 128) return launch_xinv6<T, 128, PRUNE>(in, out, a, err, st);
     }
     return false;
 }
@@ -648,7 +668,7 @@ cudaError_t launch_xinv2_slab(const FftCtx& c, const void* in, T* out, int n_rea
                               const int64_t spec[4], int lanes, cudaStream_t st)
 {
     const int M = c.plan[0].M;
-    if ((M != 256 && M != 64) || n_real > M || (n_real & 1)) return cudaErrorNotSupported;
+    if ((M != 256 && M != 128 && M != 64) || n_real > M || (n_real & 1)) return cudaErrorNotSupported;
     int lg = 0;
     while ((1 << lg) < lanes) ++lg;
     v2::X2Args a{c.tw, (int64_t)comps * zn * ny, n_real, (int)spec[0], lg, spec[1], spec[2], spec[3], n_real / 2, zn, nz, zb};
