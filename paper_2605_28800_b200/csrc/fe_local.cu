@@ -380,7 +380,10 @@ __device__ __forceinline__ void l_tma_load_4d(void* smem_dst, const CUtensorMap*
 
 // bytes of one plane slot of k_local2 (three components of a 68 x 10 tile), rounded up to the 128-byte alignment of a
 // tensor copy's destination
-template <typename T> __host__ __device__ constexpr size_t k2_slot_bytes() { return ((size_t)3 * k2Tile * sizeof(T) + 127) / 128 * 128; }
+template <typename T, bool WIDE = false> __host__ __device__ constexpr size_t k2_slot_bytes()
+{
+    return ((size_t)3 * (WIDE ? 72 : k2PX) * k2HY * sizeof(T) + 127) / 128 * 128;
+}
 
 // TMA = true (no material map, no periodic axis): a plane of the halo tile arrives as ONE tensor copy
 // (cp.async.bulk.tensor, box 68 x 10 x 1 x 3 components starting at (x0 - 2, y0 - 1, z); cells outside the sample are
@@ -401,11 +404,15 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
     // three planes ahead of their use; with a map the loader goes through registers (vacuum cells are zeroed).
     constexpr int NS = MAP ? 4 : TMA ? 6 : 5;
-    constexpr int SLOT = (int)(k2_slot_bytes<T>() / sizeof(T));             // elements between two plane slots
+    // fp32 tensor copies: a box must start on a 16-byte boundary, so the tile starts FOUR cells left of the block (x0 - 4)
+    // and is 72 wide; everywhere else two cells and 68
+    constexpr bool WIDE = TMA && sizeof(T) == 4;
+    constexpr int PX2 = WIDE ? 72 : k2PX, XO = WIDE ? 4 : 2, TL2 = PX2 * k2HY;
+    constexpr int SLOT = (int)(k2_slot_bytes<T, WIDE>() / sizeof(T));             // elements between two plane slots
     static_assert(!(TMA && MAP), "the tensor-copy loader has no vacuum masking");
-    T* tiles = reinterpret_cast<T*>(lsm);                                   // [NS][SLOT >= 3 k2Tile]
-    unsigned char* flags = lsm + (size_t)NS * SLOT * sizeof(T);             // [NS][k2Tile]
-    LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + NS * k2Tile);  // [nmat]
+    T* tiles = reinterpret_cast<T*>(lsm);                                   // [NS][SLOT >= 3 TL2]
+    unsigned char* flags = lsm + (size_t)NS * SLOT * sizeof(T);             // [NS][TL2]
+    LandauD<T>* smats = reinterpret_cast<LandauD<T>*>(flags + NS * TL2);  // [nmat]
     unsigned char* sact = reinterpret_cast<unsigned char*>(smats + a.nmat);  // [nmat]
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(
         lsm + (((size_t)(sact + a.nmat - lsm) + 7) / 8) * 8);                // [NS] "plane has landed" mbarriers of the tensor-copy loader
@@ -460,7 +467,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             bool in = true;
             if (gx < 0 || gx >= nx) { if (a.periodic[0]) gx = ((gx % nx) + nx) % nx; else in = false; }
             if (gy < 0 || gy >= ny) { if (a.periodic[1]) gy = ((gy % ny) + ny) % ny; else in = false; }
-            l_so[k] = comp * k2Tile + yy * k2PX + 2 + col;
+            l_so[k] = comp * TL2 + yy * PX2 + XO + col;
             l_go[k] = in ? gy * nx + gx : -1;
             if (in) l_ptr[k] = Y + (int64_t)comp * N + l_go[k];
         }
@@ -513,16 +520,16 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     auto store_plane = [&](int z) {
         const int slot = slot_of(z);
         T* tl = tiles + slot * SLOT;
-        unsigned char* fl = flags + slot * k2Tile;
+        unsigned char* fl = flags + slot * TL2;
 #pragma unroll
         for (int k = 0; k < k2NL; ++k) {
             if (l_so[k] < 0) continue;
             if (l_pair[k]) {
                 *reinterpret_cast<P2*>(tl + l_so[k]) = P2{pok[k][0] ? pre[k][0] : (T)0, pok[k][1] ? pre[k][1] : (T)0};
-                if (MAP && l_so[k] < k2Tile) { fl[l_so[k]] = pok[k][0]; fl[l_so[k] + 1] = pok[k][1]; }
+                if (MAP && l_so[k] < TL2) { fl[l_so[k]] = pok[k][0]; fl[l_so[k] + 1] = pok[k][1]; }
             } else {
                 tl[l_so[k]] = pok[k][0] ? pre[k][0] : (T)0;
-                if (MAP && l_so[k] < k2Tile) fl[l_so[k]] = pok[k][0];
+                if (MAP && l_so[k] < TL2) fl[l_so[k]] = pok[k][0];
             }
         }
     };
@@ -530,8 +537,8 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     auto tma_plane = [&](int z) {
         if (z > z1 || t != 0) return;
         const int slot = slot_of(z);
-        l_mbar_expect_tx(&bars[slot], (unsigned)(3 * k2Tile * sizeof(T)));
-        l_tma_load_4d(tiles + slot * SLOT, &tmap, x0 - 2, y0 - 1, z, 3 * b, &bars[slot]);
+        l_mbar_expect_tx(&bars[slot], (unsigned)(3 * TL2 * sizeof(T)));
+        l_tma_load_4d(tiles + slot * SLOT, &tmap, x0 - XO, y0 - 1, z, 3 * b, &bars[slot]);
     };
     auto tma_wait = [&](int z) { l_mbar_wait(&bars[slot_of(z)], (unsigned)(((z - z0 + 1) / NS) & 1)); };
     if (TMA && t == 0) {
@@ -564,7 +571,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     const int x = x0 + 2 * tx, y = y0 + ty;          // cells (x, y) and (x + 1, y)
     const bool inside = x < nx && y < ny;            // nx is even: both cells or none
     const int64_t rxy = (int64_t)y * nx + x;
-    const int c0 = (ty + 1) * k2PX + 2 + 2 * tx;
+    const int c0 = (ty + 1) * PX2 + XO + 2 * tx;
     const T gxfA = (T)((x > 0 || per0) + 1), gxfB = (T)(1 + (x + 2 < nx || per0));
     const T gyf = (T)((y > 0 || per1) + (y < ny - 1 || per1));
     const T G11 = (T)mem.G11, Gt = (T)mem.Gt, Gm = (T)mem.Gm, L = (T)mem.L;
@@ -594,8 +601,8 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     if (PLAIN && inside) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            cz[i] = ldp(tiles + i * k2Tile + c0);               // plane z0 - 1 sits in slot 0,
-            cc[i] = ldp(tiles + SLOT + i * k2Tile + c0);        // plane z0 in slot 1
+            cz[i] = ldp(tiles + i * TL2 + c0);               // plane z0 - 1 sits in slot 0,
+            cc[i] = ldp(tiles + SLOT + i * TL2 + c0);        // plane z0 in slot 1
         }
     }
     // slots of planes z-1, z, z+1 and the phase bits of the slots' mbarriers, carried from plane to plane (no division per plane)
@@ -623,8 +630,8 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
                     l_mbar_wait(&ebars[s3], (ephases >> s3) & 1u);
                     ephases ^= 1u << s3;
                 }
-                l_mbar_expect_tx(&bars[s3], (unsigned)(3 * k2Tile * sizeof(T)));
-                l_tma_load_4d(tiles + s3 * SLOT, &tmap, x0 - 2, y0 - 1, z + 3, 3 * b, &bars[s3]);
+                l_mbar_expect_tx(&bars[s3], (unsigned)(3 * TL2 * sizeof(T)));
+                l_tma_load_4d(tiles + s3 * SLOT, &tmap, x0 - XO, y0 - 1, z + 3, 3 * b, &bars[s3]);
             }
         } else {
             asm volatile("cp.async.wait_group 1;\n" ::);     // planes <= z+1 have landed
@@ -641,14 +648,14 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
         const T* m0 = tiles + sm1 * SLOT;           // plane z-1
         const T* c = tiles + s00 * SLOT;            // plane z
         const T* p1 = tiles + sp1 * SLOT;           // plane z+1
-        const unsigned char* fm = flags + sm1 * k2Tile;
-        const unsigned char* fc = flags + s00 * k2Tile;
-        const unsigned char* fp = flags + sp1 * k2Tile;
+        const unsigned char* fm = flags + sm1 * TL2;
+        const unsigned char* fc = flags + s00 * TL2;
+        const unsigned char* fp = flags + sp1 * TL2;
         const bool actA = !MAP || fc[c0], actB = !MAP || fc[c0 + 1];
         T EA[3] = {0, 0, 0}, EB[3] = {0, 0, 0};
         P2 pc[3];
 #pragma unroll
-        for (int i = 0; i < 3; ++i) pc[i] = PLAIN ? cc[i] : ldp(c + i * k2Tile + c0);
+        for (int i = 0; i < 3; ++i) pc[i] = PLAIN ? cc[i] : ldp(c + i * TL2 + c0);
         if (terms & 1u) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -668,19 +675,19 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             // number of existing neighbours per axis (a missing neighbour holds 0 in the tile)
             const T nzg = (T)((z > 0 || per2) + (z < nz - 1 || per2));
             const T nxA = MAP ? (T)(fc[c0 - 1] + fc[c0 + 1]) : gxfA, nxB = MAP ? (T)(fc[c0] + fc[c0 + 2]) : gxfB;
-            const T nyA = MAP ? (T)(fc[c0 - k2PX] + fc[c0 + k2PX]) : gyf;
-            const T nyB = MAP ? (T)(fc[c0 + 1 - k2PX] + fc[c0 + 1 + k2PX]) : gyf;
+            const T nyA = MAP ? (T)(fc[c0 - PX2] + fc[c0 + PX2]) : gyf;
+            const T nyB = MAP ? (T)(fc[c0 + 1 - PX2] + fc[c0 + 1 + PX2]) : gyf;
             const T nzA = MAP ? (T)(fm[c0] + fp[c0]) : nzg, nzB = MAP ? (T)(fm[c0 + 1] + fp[c0 + 1]) : nzg;
             // taps shared by the bond sums and the mixed term: rows y-1 / y+1 of plane z, planes z-1 / z+1 at row y
             P2 dn[3], up[3], zm[3], zp[3];
             T lf[3], rt[3];
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
-                const T* ci = c + i * k2Tile + c0;
-                dn[i] = ldp(ci - k2PX);
-                up[i] = ldp(ci + k2PX);
-                zm[i] = PLAIN ? cz[i] : ldp(m0 + i * k2Tile + c0);
-                zp[i] = ldp(p1 + i * k2Tile + c0);
+                const T* ci = c + i * TL2 + c0;
+                dn[i] = ldp(ci - PX2);
+                up[i] = ldp(ci + PX2);
+                zm[i] = PLAIN ? cz[i] : ldp(m0 + i * TL2 + c0);
+                zp[i] = ldp(p1 + i * TL2 + c0);
                 if (PLAIN) { cz[i] = pc[i]; cc[i] = zp[i]; }
                 lf[i] = ci[-1];
                 rt[i] = ci[2];
@@ -693,12 +700,12 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             if (MIXED) {
                 // Gm sum_{j != i} [P_j(+i+j) - P_j(+i-j) - P_j(-i+j) + P_j(-i-j)] / (4 D_i D_j); columns -1 .. +2 around cell A
                 const T* cxp = c + c0;
-                const T* cyp = c + k2Tile + c0;
-                const T* czm = m0 + 2 * k2Tile + c0;
-                const T* czp = p1 + 2 * k2Tile + c0;
+                const T* cyp = c + TL2 + c0;
+                const T* czm = m0 + 2 * TL2 + c0;
+                const T* czp = p1 + 2 * TL2 + c0;
                 // xy: Py and Px on rows y+-1
-                const T yul = cyp[k2PX - 1], yur = cyp[k2PX + 2], ydl = cyp[-k2PX - 1], ydr = cyp[-k2PX + 2];
-                const T xul = cxp[k2PX - 1], xur = cxp[k2PX + 2], xdl = cxp[-k2PX - 1], xdr = cxp[-k2PX + 2];
+                const T yul = cyp[PX2 - 1], yur = cyp[PX2 + 2], ydl = cyp[-PX2 - 1], ydr = cyp[-PX2 + 2];
+                const T xul = cxp[PX2 - 1], xur = cxp[PX2 + 2], xdl = cxp[-PX2 - 1], xdr = cxp[-PX2 + 2];
                 EA[0] += qxy * (up[1].b - dn[1].b - yul + ydl);
                 EB[0] += qxy * (yur - ydr - up[1].a + dn[1].a);
                 EA[1] += qxy * (up[0].b - dn[0].b - xul + xdl);
@@ -713,10 +720,10 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
                 EA[2] += qxz * (zp[0].b - zm[0].b - xpl + xml);
                 EB[2] += qxz * (xpr - xmr - zp[0].a + zm[0].a);
                 // yz: Pz and Py on planes z+-1 at rows y+-1
-                const P2 zpu = ldp(czp + k2PX), zpd = ldp(czp - k2PX), zmu = ldp(czm + k2PX), zmd = ldp(czm - k2PX);
-                const T* cym = m0 + k2Tile + c0;
-                const T* cyq = p1 + k2Tile + c0;
-                const P2 ypu = ldp(cyq + k2PX), ypd = ldp(cyq - k2PX), ymu = ldp(cym + k2PX), ymd = ldp(cym - k2PX);
+                const P2 zpu = ldp(czp + PX2), zpd = ldp(czp - PX2), zmu = ldp(czm + PX2), zmd = ldp(czm - PX2);
+                const T* cym = m0 + TL2 + c0;
+                const T* cyq = p1 + TL2 + c0;
+                const P2 ypu = ldp(cyq + PX2), ypd = ldp(cyq - PX2), ymu = ldp(cym + PX2), ymd = ldp(cym - PX2);
                 EA[1] += qyz * (zpu.a - zmu.a - zpd.a + zmd.a);
                 EB[1] += qyz * (zpu.b - zmu.b - zpd.b + zmd.b);
                 EA[2] += qyz * (ypu.a - ypd.a - ymu.a + ymd.a);
@@ -784,15 +791,15 @@ template <typename T> static bool make_state_map(const LocalArgs& a, CUtensorMap
         tried = true;
     }
     if (!enc) return false;
-    // fp64 only: the box starts two cells left of the tile (x0 - 2), 16 bytes in fp64 but 8 in fp32, and the copy engine
-    // raised an illegal-instruction fault on the 8-byte-aligned start on B200; fp32 keeps the cp.async loader
-    if (sizeof(T) != 8) return false;
+    // the box starts two cells left of the tile in fp64 (x0 - 2: 16 bytes) and four in fp32 (an 8-byte-aligned start raised
+    // an illegal-instruction fault in the copy engine on B200), where it is 72 cells wide
+    const cuuint32_t bx = sizeof(T) == 8 ? k2PX : 72;
     const cuuint64_t nx = a.n[0], ny = a.n[1], nz = a.n[2];
-    if ((nx * sizeof(T)) % 16 || nx < (cuuint64_t)k2PX || ny < (cuuint64_t)k2HY) return false;
+    if ((nx * sizeof(T)) % 16 || nx < (cuuint64_t)bx || ny < (cuuint64_t)k2HY) return false;
     if (reinterpret_cast<uintptr_t>(a.Y) % 16) return false;
     const cuuint64_t dims[4] = {nx, ny, nz, (cuuint64_t)3 * a.batch};
     const cuuint64_t strides[3] = {nx * sizeof(T), nx * ny * sizeof(T), nx * ny * nz * sizeof(T)};
-    const cuuint32_t box[4] = {(cuuint32_t)k2PX, (cuuint32_t)k2HY, 1, 3};
+    const cuuint32_t box[4] = {bx, (cuuint32_t)k2HY, 1, 3};
     const cuuint32_t es[4] = {1, 1, 1, 1};
     const CUresult r = enc(out, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
                            const_cast<void*>(a.Y), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -823,7 +830,9 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
     memset(&tmap, 0, sizeof(tmap));
     const bool tma = two && !a.map && !(a.periodic[0] | a.periodic[1] | a.periodic[2]) && make_state_map<T>(a, &tmap);
     const int ns = a.map ? 4 : tma ? 6 : 5;         // ring slots of k_local2
-    const size_t smem = two ? (size_t)ns * k2_slot_bytes<T>() + ns * k2Tile + (size_t)a.nmat * (sizeof(LandauD<T>) + 1) + 8 + 2 * ns * 8
+    const bool wide = tma && sizeof(T) == 4;      // fp32 tensor copies: 72-wide tiles (see k_local2)
+    const size_t slot_bytes = wide ? k2_slot_bytes<T, true>() : k2_slot_bytes<T>();
+    const size_t smem = two ? (size_t)ns * slot_bytes + ns * (wide ? 72 * k2HY : k2Tile) + (size_t)a.nmat * (sizeof(LandauD<T>) + 1) + 8 + 2 * ns * 8
                             : (size_t)4 * 3 * kTile * sizeof(T) + 4 * kTile + 8 + (size_t)a.nmat * (sizeof(LandauD<T>) + 1);
     static PerDevice<int> cache;
     int& configured = cache.here();
