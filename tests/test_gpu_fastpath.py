@@ -226,6 +226,8 @@ def test_no_write_outside_the_caller_buffers(fe, n, periodic, images, dtype):
     ((36, 140, 70), (0, 0, 0), (0, 0, 0)),        # Mc = 64, bulk-copy y pass (512, 140 data rows), Mz = 256 (70 data rows)
     ((64, 36, 24), (1, 0, 0), (1, 0, 0)),         # periodic power-of-two x, open y and z of arbitrary length
     ((100, 64, 12), (0, 1, 0), (0, 1, 0)),        # Mc = 128 (100 reals per row), periodic y, generic z
+    ((100, 64, 40), (0, 0, 0), (0, 0, 0)),        # tiled layouts, barrier-free x kernels at Mc = 128 with 100 of 128 reals per row
+    ((40, 32, 20), (0, 0, 0), (0, 0, 0)),         # ... and at Mc = 64 with 40 of 64
 ])
 def test_open_axes_of_arbitrary_length(fe, n, periodic, images):
     """Open axes need not be powers of two (the paper's own grids are 128 x 128 x 36, 80 x 80 x 80 ...): they are
