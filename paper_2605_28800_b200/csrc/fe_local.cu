@@ -611,6 +611,12 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     unsigned ephases = 0u;                           // thread 0: phase bits of the release mbarriers
     int64_t r = (int64_t)z0 * nxy + rxy;             // cell pair (x, y, z) of this thread
     for (int z = z0; z < z1; ++z, r += nxy, sm1 = s00, s00 = sp1, sp1 = (sp1 + 1 == NS ? 0 : sp1 + 1)) {
+        // E_elec of this plane: requested before the wait for the next halo plane, consumed after the stencil
+        P2 ec[3] = {{0, 0}, {0, 0}, {0, 0}};
+        if (Ee && inside) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) ec[i] = ldp(Ee + i * N + r);
+        }
         if (MAP) {
             store_plane(z + 1);
             __syncthreads();
@@ -639,12 +645,6 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             async_plane(z + 3);                              // into the slot of plane z-2 (commits a group)
         }
         if (!inside) continue;
-        // E_elec of this plane: requested here, consumed after the stencil
-        P2 ec[3] = {{0, 0}, {0, 0}, {0, 0}};
-        if (Ee) {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) ec[i] = ldp(Ee + i * N + r);
-        }
         const T* m0 = tiles + sm1 * SLOT;           // plane z-1
         const T* c = tiles + s00 * SLOT;            // plane z
         const T* p1 = tiles + sp1 * SLOT;           // plane z+1
