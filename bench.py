@@ -301,8 +301,11 @@ def run_cuda(args):
     cdom = ctr.get(dom) if isinstance(ctr.get(dom), dict) else {}
     traffic = cdom.get("dram_bytes") if cdom else (ctr.get(dom) if not isinstance(ctr.get(dom), dict) else None)
     # kernel that serves the profile slot on the size-specialised path (every bench workload but cfg1 takes it)
-    fast_names = {"xfwd": "k6_xfwd" if (args.dtype == "f64" and int(w.n[0]) == 256) else "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>",
-                  "xinv": "k6_xinv" if (args.dtype == "f64" and int(w.n[0]) == 256) else "k2_xinv",
+    # barrier-free x kernels: padded half length 256 (fp64, fp32) or 128 / 64 (fp64) on an open x axis
+    mxh = padded_dims(w)[0] // 2
+    k6 = (not w.periodic[0]) and (mxh == 256 or (args.dtype == "f64" and mxh in (64, 128)))
+    fast_names = {"xfwd": "k6_xfwd" if k6 else "k2_xfwd", "yfwd": "k4_axis<-1>", "zmul": "k2_zmul", "yinv": "k4_axis<+1>",
+                  "xinv": "k6_xinv" if k6 else "k2_xinv",
                   "local": "k_local2", "xyfwd": "k_xyfwd", "xyinv": "k_xyinv"}
     generic = args.workload == "cfg1"
     # which roofline binds the dominant kernel: the largest of its fractions of the three measured unit peaks
