@@ -392,13 +392,16 @@ template <typename T, bool WIDE = false> __host__ __device__ constexpr size_t k2
 // base, no folded stage combination, no raw-k output) -- the runtime switches of the epilogue become compile-time constants,
 // which frees the registers their pointers and flags hold and with them the per-plane recomputation of loop invariants:
 //   EPI 1: baseY == Y, no accumulator (Euler);  2: baseY == Y, accumulator (first stage of Heun / RK4);
-//   EPI 3: baseY != Y, no accumulator (last stage of Heun / RK4);  4: baseY != Y, accumulator (RK4 stages 2 and 3).
-// EPI 0 is the general epilogue (fe_rhs, AB3M2, RK45, partial term sets).
+//   EPI 3: baseY != Y, no accumulator (last stage of Heun / RK4);  4: baseY != Y, accumulator (RK4 stages 2 and 3);
+//   EPI 5: baseY == Y, raw k written, two folded terms (AB3M2 predictor with history);  6: baseY != Y, one folded term
+//   (AB3M2 corrector).
+// EPI 0 is the general epilogue (fe_rhs, RK45, the first AB3M2 steps, partial term sets).
 template <typename T, bool MAP, bool MIXED, bool TMA = false, int EPI = 0>
 __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr bool PLAIN = EPI != 0;                 // specialised epilogue
-    constexpr bool BASEY = EPI == 1 || EPI == 2, ACC = EPI == 2 || EPI == 4;
+    constexpr bool BASEY = EPI == 1 || EPI == 2 || EPI == 5, ACC = EPI == 2 || EPI == 4, KOUT = EPI == 5;
+    constexpr int NLIN = EPI == 5 ? 2 : EPI == 6 ? 1 : 0;        // folded terms of a specialised epilogue
     static_assert(!(PLAIN && MAP), "the specialised epilogues have no material map");
     extern __shared__ __align__(128) unsigned char lsm[];
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
@@ -588,7 +591,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
     const T* ai = (ACC || (!PLAIN && a.accOut)) ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
     T* ao = (ACC || (!PLAIN && a.accOut)) ? static_cast<T*>(a.accOut) + (int64_t)b * 3 * N : nullptr;
-    const int nlin = PLAIN ? 0 : a.nlin;
+    const int nlin = PLAIN ? NLIN : a.nlin;
     const LandauD<T> lc0 = smats[0];
     auto ldp = [](const T* q) { return *reinterpret_cast<const P2*>(q); };
 
@@ -744,7 +747,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             if (actA) kA[i] = L * EA[i];
             if (actB) kB[i] = L * EB[i];
         }
-        if (!PLAIN && a.kOut) {
+        if (KOUT || (!PLAIN && a.kOut)) {
             T* ko = static_cast<T*>(a.kOut) + (int64_t)b * 3 * N;
 #pragma unroll
             for (int i = 0; i < 3; ++i) *reinterpret_cast<P2*>(ko + i * N + r) = P2{kA[i], kB[i]};
@@ -856,6 +859,8 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             attr(m, tm, std::integral_constant<int, 2>{});
             attr(m, tm, std::integral_constant<int, 3>{});
             attr(m, tm, std::integral_constant<int, 4>{});
+            attr(m, tm, std::integral_constant<int, 5>{});
+            attr(m, tm, std::integral_constant<int, 6>{});
         };
         a2(std::true_type{}, std::true_type{});
         a2(std::true_type{}, std::false_type{});
@@ -870,8 +875,11 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             else k_local2<T, true, false><<<grid, 256, smem, st>>>(a, tmap);
         } else {
             // a stage of Euler / Heun / RK4 with all four terms: one of the specialised epilogues (see k_local2)
-            const bool spec = a.terms == 15u && a.Eelec && a.baseY && !a.kOut && a.nlin == 0;
-            const int epi = !spec ? 0 : a.baseY == a.Y ? (a.accOut ? 2 : 1) : (a.accOut ? 4 : 3);
+            const bool full = a.terms == 15u && a.Eelec && a.baseY;
+            int epi = 0;
+            if (full && !a.kOut && a.nlin == 0) epi = a.baseY == a.Y ? (a.accOut ? 2 : 1) : (a.accOut ? 4 : 3);
+            else if (full && a.kOut && a.nlin == 2 && a.baseY == a.Y && !a.accOut) epi = 5;
+            else if (full && !a.kOut && a.nlin == 1 && a.baseY != a.Y && !a.accOut) epi = 6;
             auto go = [&](auto m, auto tm, auto ep) {
                 k_local2<T, false, decltype(m)::value, decltype(tm)::value, decltype(ep)::value><<<grid, 256, smem, st>>>(a, tmap);
             };
@@ -881,6 +889,8 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
                     case 2: go(m, tm, std::integral_constant<int, 2>{}); break;
                     case 3: go(m, tm, std::integral_constant<int, 3>{}); break;
                     case 4: go(m, tm, std::integral_constant<int, 4>{}); break;
+                    case 5: go(m, tm, std::integral_constant<int, 5>{}); break;
+                    case 6: go(m, tm, std::integral_constant<int, 6>{}); break;
                     default: go(m, tm, std::integral_constant<int, 0>{}); break;
                 }
             };
