@@ -554,8 +554,17 @@ static bool launch_xinv6(const void* in, void* out, const X2Args& a, cudaError_t
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) { sms = 0; *err = e; return true; }
     }
-    int per = 0;        // the shared-memory size depends on the layout (G): ask every time (a cheap host-side query)
-    if ((*err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xinv<T, M, PRUNE>, 256, smem)) != cudaSuccess) return true;
+    // blocks per SM: depends on the shared-memory size, i.e. on the layout (G); asked again only when that changes
+    struct Occ { size_t smem = 0; int per = 0; };
+    static PerDevice<Occ> occ;
+    Occ& o = occ.here();
+    if (o.smem != smem) {
+        int per = 0;
+        if ((*err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k6_xinv<T, M, PRUNE>, 256, smem)) != cudaSuccess) return true;
+        o.smem = smem;
+        o.per = per;
+    }
+    const int per = o.per;
     const int nblocks = sms * (per > 0 ? per : 1);
     const int ngroups = nplanes * (a.ny / C::ROWS);
     const int grid = ngroups < nblocks ? ngroups : nblocks;
