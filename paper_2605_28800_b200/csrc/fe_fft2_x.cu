@@ -237,6 +237,8 @@ __global__ void __launch_bounds__(256, 2) k6_xinv(T* __restrict__ out, X2Args a,
         int plane = grp / gpp;
         const int y0 = (grp - plane * gpp) * ROWS;
         if (a.pl_n) plane = (plane / a.pl_n) * a.pl_full + a.pl_off + plane % a.pl_n;
+        // the warp's generic-proxy reads and exchange writes of the buffer are ordered before the copy engine's writes
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(x6_smem_u32(bar)), "r"(bytes) : "memory");
         asm volatile(
             "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];\n" ::"r"(
