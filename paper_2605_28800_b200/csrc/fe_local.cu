@@ -394,7 +394,7 @@ template <typename T, bool WIDE = false> __host__ __device__ constexpr size_t k2
 //   EPI 1: baseY == Y, no accumulator (Euler);  2: baseY == Y, accumulator (first stage of Heun / RK4);
 //   EPI 3: baseY != Y, no accumulator (last stage of Heun / RK4);  4: baseY != Y, accumulator (RK4 stages 2 and 3);
 //   EPI 5: baseY == Y, raw k written, two folded terms (AB3M2 predictor with history);  6: baseY != Y, one folded term
-//   (AB3M2 corrector).
+//   (AB3M2 corrector);  7: no base, no accumulator: the plain right-hand side of fe_rhs.
 // EPI 0 is the general epilogue (fe_rhs, RK45, the first AB3M2 steps, partial term sets).
 template <typename T, bool MAP, bool MIXED, bool TMA = false, int EPI = 0>
 __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_constant__ CUtensorMap tmap)
@@ -402,6 +402,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
     constexpr bool PLAIN = EPI != 0;                 // specialised epilogue
     constexpr bool BASEY = EPI == 1 || EPI == 2 || EPI == 5, ACC = EPI == 2 || EPI == 4, KOUT = EPI == 5;
     constexpr int NLIN = EPI == 5 ? 2 : EPI == 6 ? 1 : 0;        // folded terms of a specialised epilogue
+    constexpr bool NOBASE = EPI == 7;
     static_assert(!(PLAIN && MAP), "the specialised epilogues have no material map");
     extern __shared__ __align__(128) unsigned char lsm[];
     // ring of NS plane slots.  Without a material map the planes arrive by cp.async (zero fill outside the sample)
@@ -586,7 +587,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
             ex2 = (T)(mem.Eext[2] + mem.wamp[2] * wv);
     const uint32_t terms = PLAIN ? 15u : a.terms;
     const T* Ee = PLAIN || ((terms & 4u) && a.Eelec) ? static_cast<const T*>(a.Eelec) + (int64_t)b * 3 * N : nullptr;
-    const T* base = BASEY ? Y : (PLAIN || a.baseY) ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
+    const T* base = BASEY ? Y : NOBASE ? nullptr : (PLAIN || a.baseY) ? static_cast<const T*>(a.baseY) + (int64_t)b * 3 * N : nullptr;
     const bool base_is_Y = BASEY || (!PLAIN && a.baseY == a.Y);
     T* Yout = static_cast<T*>(a.Yout) + (int64_t)b * 3 * N;
     const T* ai = (ACC || (!PLAIN && a.accOut)) ? static_cast<const T*>(a.accIn) + (int64_t)b * 3 * N : nullptr;
@@ -755,7 +756,7 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             P2 bv = {0, 0};
-            if (PLAIN || base) {
+            if (!NOBASE && (PLAIN || base)) {
                 // Euler: the stage base is the state itself, already in the tile (vacuum cells hold their raw value in memory)
                 if (base_is_Y && actA && actB) bv = pc[i];
                 else bv = ldp(base + i * N + r);
@@ -861,6 +862,7 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             attr(m, tm, std::integral_constant<int, 4>{});
             attr(m, tm, std::integral_constant<int, 5>{});
             attr(m, tm, std::integral_constant<int, 6>{});
+            attr(m, tm, std::integral_constant<int, 7>{});
         };
         a2(std::true_type{}, std::true_type{});
         a2(std::true_type{}, std::false_type{});
@@ -877,6 +879,7 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             // a stage of Euler / Heun / RK4 with all four terms: one of the specialised epilogues (see k_local2)
             const bool full = a.terms == 15u && a.Eelec && a.baseY;
             int epi = 0;
+            if (a.terms == 15u && a.Eelec && !a.baseY && !a.kOut && a.nlin == 0 && !a.accOut) epi = 7;
             if (full && !a.kOut && a.nlin == 0) epi = a.baseY == a.Y ? (a.accOut ? 2 : 1) : (a.accOut ? 4 : 3);
             else if (full && a.kOut && a.nlin == 2 && a.baseY == a.Y && !a.accOut) epi = 5;
             else if (full && !a.kOut && a.nlin == 1 && a.baseY != a.Y && !a.accOut) epi = 6;
@@ -891,6 +894,7 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
                     case 4: go(m, tm, std::integral_constant<int, 4>{}); break;
                     case 5: go(m, tm, std::integral_constant<int, 5>{}); break;
                     case 6: go(m, tm, std::integral_constant<int, 6>{}); break;
+                    case 7: go(m, tm, std::integral_constant<int, 7>{}); break;
                     default: go(m, tm, std::integral_constant<int, 0>{}); break;
                 }
             };
