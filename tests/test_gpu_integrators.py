@@ -164,3 +164,24 @@ def test_rk45_nonfinite_state_is_refused_not_accepted(fe, bad):
         g.step_rk45(P, 0.4, 0.05, 1e-6, 1000, fi.TERM_ALL)
     assert ei.value.status == fe.FE_ENONFINITE
     g.close()
+
+
+@pytest.mark.parametrize("dtype,tol", [("f64", 1e-11), ("f32", 1e-4)])
+def test_specialised_stage_epilogues_on_the_tensor_copy_path(fe, dtype, tol):
+    """Open grid without a material map, wide enough for the tensor-copy halo tiles (72 x 16 x 8, batch 2, Gm != 0): the stages
+    of Euler, Heun, RK4 and AB3M2 (with history) and the plain right-hand side each take their own instantiation of the local
+    step (compile-time epilogue) -- every one of them against the oracle."""
+    w = fi.open_batio3("epilogues_72x16x8", (72, 16, 8), 2, dtype, 4242)
+    P0 = w.P0 if dtype == "f64" else w.P0.astype(np.float32).astype(np.float64)
+    g = fe.Grid.from_workload(w, dtype=dtype)
+    g.precompute_tensor()
+    o = orc.Oracle(oracle_problem(w, 1), elec="fft")
+    P = g.state(P0)
+    assert rel_l2(g.rhs(P, fi.TERM_ALL).cpu().numpy()[1], o.rhs(P0[1], fi.TERM_ALL)) < (1e-10 if dtype == "f64" else tol)
+    dt = 4 * w.dt
+    for integ, nsteps in ((fi.EULER, 6), (fi.HEUN, 4), (fi.RK4, 3), (fi.AB3M2, 6)):
+        P = g.state(P0)
+        g.step(P, dt, nsteps, integ, fi.TERM_ALL)
+        want = o.step_ab3m2(P0[1], dt, nsteps, fi.TERM_ALL) if integ == fi.AB3M2 else o.step(P0[1], dt, nsteps, integ, fi.TERM_ALL)
+        assert rel_l2(P.cpu().numpy()[1].astype(np.float64), want) < tol, integ
+    g.close()
