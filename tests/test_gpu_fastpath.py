@@ -40,6 +40,10 @@ def _workload(n, periodic=(0, 0, 0), images=(0, 0, 0), batch=1, seed=77):
     ((128, 64, 32), (1, 1, 0), (1, 1, 0)),       #  64    64    64p  (unpruned x, y)
     ((64, 64, 64), (0, 0, 1), (0, 0, 1)),        #  64p  128p   64   (unpruned z)
     ((256, 128, 16), (1, 1, 0), (1, 1, 0)),      # 128   128   generic
+    ((1024, 4, 4), (1, 0, 0), (1, 0, 0)),        # the largest periodic axis the ABI admits, on x (unpruned 512), ...
+    ((4, 1024, 4), (0, 1, 0), (0, 1, 0)),        # ... on y ...
+    ((4, 4, 1024), (0, 0, 1), (0, 0, 1)),        # ... and on z (generic passes)
+    ((512, 4, 4), (0, 0, 0), (0, 0, 0)),         # the largest open axis: 512 cells padded to 1024
 ])
 def test_fast_passes_against_oracle_fft(fe, n, periodic, images):
     w = _workload(n, periodic, images)
