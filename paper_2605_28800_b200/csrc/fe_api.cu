@@ -59,6 +59,7 @@ struct fe_grid {
     unsigned char* ws;
     size_t ws_bytes;
     size_t o_Kt, o_S1, o_S2, o_E, o_Y, o_ACC, o_PP, o_K[6], o_part, o_cnt, o_box, o_Sbox, total_bytes;
+    int vac0;                        // material 0 of some member is vacuum
     int opt_fuse_xy;                 // FE_OPT_FUSE_XY
     int opt_xl_slabs;                // FE_OPT_XL_SLABS
     int opt_xy_ring;                 // FE_OPT_XY_RING (0: automatic)
@@ -244,6 +245,7 @@ extern "C" fe_status fe_create_grid(const fe_grid_desc* d, fe_grid** out)
     }
     g->dirty = true;
     g->mixed = 0;
+    g->vac0 = 0;
     g->opt_fuse_xy = 0;
     g->opt_xl_slabs = 0;
     g->opt_xy_ring = 0;
@@ -508,9 +510,11 @@ static fe_status sync_params(fe_grid* g, cudaStream_t st)
     if (!g->dirty) return FE_OK;
     g->gvalid = false;               // kernel variants (mixed term) may change with the coefficients
     g->mixed = 0;
+    g->vac0 = 0;
     g->any_wave = false;
     for (int b = 0; b < B; ++b) {
         if (g->h_members[b].Gm != 0.0) g->mixed = 1;
+        if (!g->h_mats[(size_t)b * M].active) g->vac0 = 1;
         if (g->h_members[b].wave) g->any_wave = true;
     }
     FE_CUDA(cudaMemcpyAsync(g->d_mats, g->h_mats.data(), (size_t)B * M * sizeof(DevLandau), cudaMemcpyHostToDevice, st));
@@ -722,6 +726,7 @@ static fe_status stage(fe_grid* g, const T* Y, const T* baseY, T* Yout, double c
     a.terms = terms;
     a.batch = g->desc.batch;
     a.mixed = g->mixed;
+    a.vac0 = g->vac0;
     a.t = g->tstage;
     if (nslab > 1) {
         const int64_t p = q.pitch;

@@ -177,6 +177,7 @@ struct LocalArgs {
     uint32_t terms;
     int batch;
     int mixed;            // any member has Gm != 0
+    int vac0;             // material 0 of some member is vacuum (matters without a map: that member is all vacuum)
     double t;             // time at which E_ext is sampled (stage time)
     // filled by launch_local
     double id2[3];        // 1 / D_a^2

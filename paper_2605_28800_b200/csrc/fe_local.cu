@@ -93,9 +93,7 @@ struct Grid {
     {
         if ((x | y | z) < 0) { ok = false; return (T)0; }
         const int64_t r = ((int64_t)z * ny + y) * nx + x;
-        if (MAP) {
-            if (!mats[map[r]].active) { ok = false; return (T)0; }
-        }
+        if (!mats[MAP ? map[r] : 0].active) { ok = false; return (T)0; }     // (no map: every cell is material 0)
         ok = true;
         return p[c][r];
     }
@@ -239,7 +237,8 @@ __global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
         const unsigned char* fp = flags + ((z + 1) & 3) * kTile;
         const int64_t r = (int64_t)z * nxy + rxy;
         T k[3] = {0, 0, 0};
-        if (!MAP || fc[c0]) {
+        const bool act = MAP ? fc[c0] != 0 : lc0.active != 0;       // without a map every cell is material 0 (vacuum: pinned)
+        if (act) {
             const T px = c[c0], py = c[kTile + c0], pz = c[2 * kTile + c0];
             T E0 = 0, E1 = 0, E2 = 0;
             if (a.terms & 1u) {
@@ -292,7 +291,7 @@ __global__ void __launch_bounds__(256, 2) k_local(LocalArgs a)
         if (base) {
             if (base_is_Y) {
                 // the stage base is the state itself (Euler): take it from the tile; vacuum cells hold their raw value
-                if (!MAP || fc[c0]) { bv[0] = c[c0]; bv[1] = c[kTile + c0]; bv[2] = c[2 * kTile + c0]; }
+                if (act) { bv[0] = c[c0]; bv[1] = c[kTile + c0]; bv[2] = c[2 * kTile + c0]; }
                 else { bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r]; }
             } else {
                 bv[0] = base[r]; bv[1] = base[N + r]; bv[2] = base[2 * N + r];
@@ -396,9 +395,12 @@ template <typename T, bool WIDE = false> __host__ __device__ constexpr size_t k2
 //   EPI 5: baseY == Y, raw k written, two folded terms (AB3M2 predictor with history);  6: baseY != Y, one folded term
 //   (AB3M2 corrector);  7: no base, no accumulator: the plain right-hand side of fe_rhs.
 // EPI 0 is the general epilogue (fe_rhs, RK45, the first AB3M2 steps, partial term sets).
-template <typename T, bool MAP, bool MIXED, bool TMA = false, int EPI = 0>
+// VAC = true (general epilogue without a map only): material 0 of some member is vacuum, i.e. the whole member is pinned;
+// every other instantiation without a map takes all cells as active.
+template <typename T, bool MAP, bool MIXED, bool TMA = false, int EPI = 0, bool VAC = false>
 __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_constant__ CUtensorMap tmap)
 {
+    static_assert(!VAC || (!MAP && EPI == 0), "the vacuum check belongs to the general epilogue without a map");
     constexpr bool PLAIN = EPI != 0;                 // specialised epilogue
     constexpr bool BASEY = EPI == 1 || EPI == 2 || EPI == 5, ACC = EPI == 2 || EPI == 4, KOUT = EPI == 5;
     constexpr int NLIN = EPI == 5 ? 2 : EPI == 6 ? 1 : 0;        // folded terms of a specialised epilogue
@@ -655,7 +657,9 @@ __global__ void __launch_bounds__(256, 2) k_local2(LocalArgs a, const __grid_con
         const unsigned char* fm = flags + sm1 * TL2;
         const unsigned char* fc = flags + s00 * TL2;
         const unsigned char* fp = flags + sp1 * TL2;
-        const bool actA = !MAP || fc[c0], actB = !MAP || fc[c0 + 1];
+        // without a map every cell is material 0 (a vacuum material 0 pins the whole member: VAC)
+        const bool act0 = !VAC || lc0.active != 0;
+        const bool actA = MAP ? fc[c0] != 0 : act0, actB = MAP ? fc[c0 + 1] != 0 : act0;
         T EA[3] = {0, 0, 0}, EB[3] = {0, 0, 0};
         P2 pc[3];
 #pragma unroll
@@ -864,6 +868,10 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             attr(m, tm, std::integral_constant<int, 6>{});
             attr(m, tm, std::integral_constant<int, 7>{});
         };
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, true, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, true, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_local2<T, false, false, false, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim2);
         a2(std::true_type{}, std::true_type{});
         a2(std::true_type{}, std::false_type{});
         a2(std::false_type{}, std::true_type{});
@@ -879,6 +887,16 @@ template <typename T> cudaError_t launch_local(const LocalArgs& a0, cudaStream_t
             // a stage of Euler / Heun / RK4 with all four terms: one of the specialised epilogues (see k_local2)
             const bool full = a.terms == 15u && a.Eelec && a.baseY;
             int epi = 0;
+            if (a.vac0) {                  // some member is all vacuum: general epilogue with the activity check
+                if (tma) {
+                    if (a.mixed) k_local2<T, false, true, true, 0, true><<<grid, 256, smem, st>>>(a, tmap);
+                    else k_local2<T, false, false, true, 0, true><<<grid, 256, smem, st>>>(a, tmap);
+                } else {
+                    if (a.mixed) k_local2<T, false, true, false, 0, true><<<grid, 256, smem, st>>>(a, tmap);
+                    else k_local2<T, false, false, false, 0, true><<<grid, 256, smem, st>>>(a, tmap);
+                }
+                return cudaGetLastError();
+            }
             if (a.terms == 15u && a.Eelec && !a.baseY && !a.kOut && a.nlin == 0 && !a.accOut) epi = 7;
             if (full && !a.kOut && a.nlin == 0) epi = a.baseY == a.Y ? (a.accOut ? 2 : 1) : (a.accOut ? 4 : 3);
             else if (full && a.kOut && a.nlin == 2 && a.baseY == a.Y && !a.accOut) epi = 5;

@@ -241,6 +241,48 @@ def test_error_paths(fe):
     assert ei.value.status == fe.FE_ESTATE
 
 
+def test_degenerate_inputs(fe):
+    """Zero steps, the zero state, an all-vacuum sample and the smallest grid the ABI admits."""
+    import torch
+    from dataclasses import replace
+    w = fi.config1()
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    before = P.clone()
+    for integ in (fi.EULER, fi.HEUN, fi.RK4, fi.AB3M2):
+        g.step(P, w.dt, 0, integ, fi.TERM_ALL)                     # nsteps = 0: nothing happens, the clock stands still
+        assert torch.equal(P, before) and g.time() == 0.0
+    # P = 0: no Landau, gradient or electrostatic field; dP/dt = L E_ext exactly, energies zero
+    Z = torch.zeros_like(P)
+    got = g.rhs(Z, fi.TERM_ALL).cpu().numpy()[0]
+    want = orc.Oracle(oracle_problem(w)).rhs(np.zeros_like(w.P0[0]), fi.TERM_ALL)
+    assert np.array_equal(got, want)
+    assert np.all(g.energy(Z) == 0.0)
+    g.close()
+    # all cells vacuum: the state is pinned, the right-hand side is zero whatever the terms
+    for wv in (fi.config1(), fi.open_batio3("vacuum_64x8x8", (64, 8, 8), 1, "f64", 7),      # one- and two-cell local kernels,
+               fi.open_batio3("vacuum_72x16x8", (72, 16, 8), 1, "f64", 8)):                    # tensor-copy tiles
+        wv.materials = [[replace(wv.materials[0][0], active=0)]]
+        gv = fe.Grid.from_workload(wv)
+        gv.precompute_tensor()
+        Pv = gv.state(wv.P0)
+        assert not gv.rhs(Pv, fi.TERM_ALL).any()
+        for integ in (fi.EULER, fi.RK4):
+            gv.step(Pv, wv.dt, 3, integ, fi.TERM_ALL)
+            assert torch.equal(Pv, gv.state(wv.P0))
+        assert np.all(gv.energy(Pv)[:, :5] == 0.0)
+        gv.close()
+    # the smallest grid: 4 x 4 x 4 periodic and 2 x 2 x 2 open, against the direct sum
+    for n, per, img in (((4, 4, 4), (1, 1, 1), (2, 2, 2)), ((2, 2, 2), (0, 0, 0), (0, 0, 0))):
+        ws = workload_from_random(97, n, per, img, batch=1)
+        gs = fe.Grid.from_workload(ws)
+        gs.precompute_tensor()
+        os_ = orc.Oracle(oracle_problem(ws), elec="direct")
+        assert rel_l2(gs.rhs(gs.state(ws.P0), fi.TERM_ALL).cpu().numpy()[0], os_.rhs(ws.P0[0], fi.TERM_ALL)) < TOL_RHS64, n
+        gs.close()
+
+
 @pytest.mark.parametrize("integ", [fi.EULER, fi.HEUN, fi.RK4])
 def test_graph_replay_equals_eager_stepping(fe, integ):
     """fe_step(n) with n large replays a CUDA graph of one unit of steps; it must give bit-identical results to n single
