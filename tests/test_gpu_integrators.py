@@ -166,12 +166,15 @@ def test_rk45_nonfinite_state_is_refused_not_accepted(fe, bad):
     g.close()
 
 
-@pytest.mark.parametrize("dtype,tol", [("f64", 1e-11), ("f32", 1e-4)])
-def test_specialised_stage_epilogues_on_the_tensor_copy_path(fe, dtype, tol):
+@pytest.mark.parametrize("dtype,tol,gm0", [("f64", 1e-11, False), ("f32", 1e-4, False), ("f64", 1e-11, True)])
+def test_specialised_stage_epilogues_on_the_tensor_copy_path(fe, dtype, tol, gm0):
     """Open grid without a material map, wide enough for the tensor-copy halo tiles (72 x 16 x 8, batch 2, Gm != 0): the stages
     of Euler, Heun, RK4 and AB3M2 (with history) and the plain right-hand side each take their own instantiation of the local
     step (compile-time epilogue) -- every one of them against the oracle."""
     w = fi.open_batio3("epilogues_72x16x8", (72, 16, 8), 2, dtype, 4242)
+    if gm0:                                  # Gm = G12 + G44 - G'44 = 0: the instantiations without the mixed-derivative taps
+        from dataclasses import replace
+        w.globals_ = [replace(q, G12=q.G44p - q.G44) for q in w.globals_]
     P0 = w.P0 if dtype == "f64" else w.P0.astype(np.float32).astype(np.float64)
     g = fe.Grid.from_workload(w, dtype=dtype)
     g.precompute_tensor()
