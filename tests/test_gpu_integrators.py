@@ -188,3 +188,55 @@ def test_specialised_stage_epilogues_on_the_tensor_copy_path(fe, dtype, tol, gm0
         want = o.step_ab3m2(P0[1], dt, nsteps, fi.TERM_ALL) if integ == fi.AB3M2 else o.step(P0[1], dt, nsteps, integ, fi.TERM_ALL)
         assert rel_l2(P.cpu().numpy()[1].astype(np.float64), want) < tol, integ
     g.close()
+
+
+def test_wave_static_field_and_eighth_order_terms_on_the_tensor_copy_path(fe):
+    """The same grid with everything the stage epilogues sample per member: a static E_ext, a sinusoidal one at the stage
+    times, a clock that does not start at zero, non-zero 8th-order Landau slots -- and the adaptive RK45 on top (generic
+    epilogue with folded stage combinations), decision by decision."""
+    from dataclasses import replace
+    w = fi.open_batio3("epilogues_72x16x8", (72, 16, 8), 2, "f64", 4243)
+    w.materials = [[replace(m[0], a1111=0.3 * abs(m[0].a111), a1112=-0.2 * abs(m[0].a111), a1122=0.1 * abs(m[0].a111),
+                            a1123=0.25 * abs(m[0].a111))] for m in w.materials]
+    fields = [(0.02, -0.01, 0.03), (-0.015, 0.02, 0.01)]
+    waves = [((0.03, -0.02, 0.05), 7.0, 0.4), ((-0.01, 0.06, 0.02), 3.0, -1.1)]
+    w.globals_ = [replace(q, E_ext=fields[b]) for b, q in enumerate(w.globals_)]
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    oracles = []
+    for b in range(2):
+        g.set_external_wave(b, *waves[b])
+        o = orc.Oracle(oracle_problem(w, b), elec="fft")
+        o.set_wave(*waves[b])
+        oracles.append(o)
+    t0, dt = 0.37, 4 * w.dt
+    g.set_time(t0)
+    P = g.state(w.P0)
+    got = g.rhs(P).cpu().numpy()
+    for b in range(2):
+        assert rel_l2(got[b], oracles[b].rhs(w.P0[b], fi.TERM_ALL, t0)) < 1e-10
+    for integ, name in ((fi.EULER, "euler"), (fi.HEUN, "heun"), (fi.RK4, "rk4"), (fe.FE_AB3M2, "ab3m2")):
+        g.set_time(t0)
+        P = g.state(w.P0)
+        g.step(P, dt, 5, integ, fi.TERM_ALL)
+        for b in range(2):
+            o = oracles[b]
+            want = (o.step_ab3m2(w.P0[b], dt, 5, fi.TERM_ALL, t0=t0) if name == "ab3m2"
+                    else o.step(w.P0[b], dt, 5, integ, fi.TERM_ALL, t0=t0))
+            assert rel_l2(P.cpu().numpy()[b], want) < 1e-11, (name, b)
+    g.close()
+    # adaptive RK45, one member so that the accept / reject decisions can be compared one by one
+    w1 = fi.open_batio3("epilogues_72x16x8", (72, 16, 8), 1, "f64", 4244)
+    w1.globals_ = [replace(w1.globals_[0], E_ext=fields[0])]
+    g1 = fe.Grid.from_workload(w1)
+    g1.precompute_tensor()
+    g1.set_external_wave(0, *waves[0])
+    o1 = orc.Oracle(oracle_problem(w1), elec="fft")
+    o1.set_wave(*waves[0])
+    g1.set_time(t0)
+    P1 = g1.state(w1.P0)
+    st = g1.step_rk45(P1, 0.03, 0.02, 1e-8, 200, fi.TERM_ALL)
+    want, so = o1.step_rk45(w1.P0[0], 0.03, 0.02, 1e-8, 200, fi.TERM_ALL, t0=t0)
+    assert (st["accepted"], st["rejected"]) == (so["accepted"], so["rejected"]) and st["accepted"] >= 2
+    assert rel_l2(P1.cpu().numpy()[0], want) < 1e-11
+    g1.close()
