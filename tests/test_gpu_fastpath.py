@@ -232,6 +232,7 @@ def test_no_write_outside_the_caller_buffers(fe, n, periodic, images, dtype):
     ((100, 64, 12), (0, 1, 0), (0, 1, 0)),        # Mc = 128 (100 reals per row), periodic y, generic z
     ((100, 64, 40), (0, 0, 0), (0, 0, 0)),        # tiled layouts, barrier-free x kernels at Mc = 128 with 100 of 128 reals per row
     ((40, 32, 20), (0, 0, 0), (0, 0, 0)),         # ... and at Mc = 64 with 40 of 64
+    ((130, 6, 6), (0, 0, 0), (0, 0, 0)),          # Mc = 256 beside generic y and z: row-major spectra, 108 rows (not a multiple of 16)
 ])
 def test_open_axes_of_arbitrary_length(fe, n, periodic, images):
     """Open axes need not be powers of two (the paper's own grids are 128 x 128 x 36, 80 x 80 x 80 ...): they are
