@@ -341,3 +341,30 @@ def test_x_inverse_hands_e_elec_to_the_local_step_slab_by_slab(fe, n, batch, sla
         g.step(Pb, w.dt, nst, integ, fi.TERM_ALL)
         assert np.array_equal(Pa.cpu().numpy(), Pb.cpu().numpy())
     g.close()
+
+
+def test_calls_on_a_side_stream(fe):
+    """Every call takes the caller's stream (the binding passes torch's current stream): right-hand side, steps under graph
+    replay, energies and the no-allocation energy entry point on a non-default stream give what the default stream gives."""
+    import torch
+    w = _workload((128, 32, 16))
+    g = fe.Grid.from_workload(w)
+    g.precompute_tensor()
+    P = g.state(w.P0)
+    ref_rhs = g.rhs(P, fi.TERM_ALL).clone()
+    Pr = g.state(w.P0)
+    g.step(Pr, w.dt, 30, fi.EULER, fi.TERM_ALL)
+    ref_e = g.energy(Pr)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        got_rhs = g.rhs(P, fi.TERM_ALL).clone()
+        Ps = g.state(w.P0)
+        g.step(Ps, w.dt, 30, fi.EULER, fi.TERM_ALL)
+        got_e = g.energy(Ps)
+        out = torch.empty((1, 8), dtype=torch.float64, device=P.device)
+        g.energy_noalloc(Ps, out, fi.TERM_ALL)
+    side.synchronize()
+    assert torch.equal(got_rhs, ref_rhs) and torch.equal(Ps, Pr)
+    assert np.array_equal(got_e, ref_e) and np.array_equal(out.cpu().numpy(), ref_e)
+    g.close()
