@@ -340,6 +340,18 @@ def test_x_inverse_hands_e_elec_to_the_local_step_slab_by_slab(fe, n, batch, sla
         Pb = g.state(w.P0)
         g.step(Pb, w.dt, nst, integ, fi.TERM_ALL)
         assert np.array_equal(Pa.cpu().numpy(), Pb.cpu().numpy())
+    # both options at once: fused x + y forward pass and the slab hand-over
+    if n[1] in (128, 256):
+        g.set_option(fe.FE_OPT_XL_SLABS, slabs)
+        g.set_option(fe.FE_OPT_FUSE_XY, 1)
+        Pa = g.state(w.P0)
+        g.step(Pa, w.dt, 6, fi.EULER, fi.TERM_ALL)
+        g.set_option(fe.FE_OPT_XL_SLABS, 0)
+        g.set_option(fe.FE_OPT_FUSE_XY, 0)
+        Pb = g.state(w.P0)
+        g.step(Pb, w.dt, 6, fi.EULER, fi.TERM_ALL)
+        assert rel_l2(Pa.cpu().numpy(), Pb.cpu().numpy()) < 1e-13
+        assert g.get_option(fe.FE_OPT_XY_TIMEOUTS) == 0
     g.close()
 
 
