@@ -92,6 +92,17 @@ def test_two_cell_local_kernel_heterogeneous(fe, n, periodic, images):
         want = o.step(w.P0[1], 1e-2, 3, integ, fi.TERM_ALL)
         assert rel_l2(Pd.cpu().numpy()[1], want) < 1e-12, integ
     g.close()
+    # the same problem in fp32 (material map, vacuum, periodic wrap in the register loaders of the two-cell kernel)
+    g = fe.Grid.from_workload(w, dtype="f32")
+    g.precompute_tensor()
+    P32 = w.P0.astype(np.float32)
+    got = g.rhs(g.state(P32), fi.TERM_ALL).cpu().numpy()[1].astype(np.float64)
+    assert rel_l2(got, o.rhs(P32[1].astype(np.float64), fi.TERM_ALL)) < TOL32
+    assert np.all(got[:, o.p.active == 0] == 0.0)
+    Pd = g.state(P32)
+    g.step(Pd, 1e-2, 3, fi.RK4, fi.TERM_ALL)
+    assert rel_l2(Pd.cpu().numpy()[1].astype(np.float64), o.step(P32[1].astype(np.float64), 1e-2, 3, fi.RK4, fi.TERM_ALL)) < TOL32
+    g.close()
 
 
 def test_fast_passes_batch_and_fp32(fe):
